@@ -1,0 +1,408 @@
+"""Pins P1-P14: the oracle against closed forms, invariants, library
+routines and brute force — never against itself and never against the CUDA path.
+
+The paper prints no worked example (PAPER.md has no equations or numeric fixtures), so every
+pin is a mathematical one; each is chosen so that a plausible mistake (dropped term, wrong
+sign or index, transposed axis, off-by-half lattice) fails at least one of them.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle as O
+import workload as W
+
+RNG = np.random.default_rng(20241104)
+
+
+def noise_cube(nx, ny, nz, seed=11):
+    return W.make_cube(W.Recipe(nx, ny, nz, seed=seed))
+
+
+KS = 255.0 / 256.0
+
+
+def ramp_alpha_tf(amax=0.5):
+    """Entries i/256-based so every entry is exact in float32 and the table lerp IS the line:
+    rgb(u) = (KS*u, 1-KS*u, 0.25), alpha(u) = amax*KS*u   (amax a power of two)."""
+    w = np.arange(256, dtype=np.float64) / 256.0
+    t = np.stack([w, 1 - w, np.full_like(w, 0.25), amax * w], axis=1)
+    assert np.array_equal(t.astype(np.float32).astype(np.float64), t)
+    return t.astype(np.float32)
+
+
+def const_tf(rgba):
+    return np.tile(np.asarray(rgba, dtype=np.float32), (256, 1))
+
+
+# --------------------------------------------------------------------------- P1 / P10
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("sign", [+1, -1])
+def test_p1_axis_aligned_ortho_mip_is_column_max(axis, sign):
+    v = noise_cube(13, 9, 17)                       # shape (nz, ny, nx)
+    cam = W.ortho_axis_camera((13, 9, 17), axis, sign, step=1.0)
+    r = O.render(v, cam, O.MIP)
+    want = v.max(axis={0: 2, 1: 1, 2: 0}[axis])     # image[j, i]: i <-> u axis, j <-> v axis
+    assert r.image.shape == want.shape
+    assert np.array_equal(r.image, want)            # bit-exact, incl. the last voxel (i0=n-2, f=1)
+    assert np.all(r.K == (13, 9, 17)[axis])
+    r64 = O.render(v, cam, O.MIP, precision=O.F64)
+    assert np.array_equal(r64.image, want)
+
+
+def test_p1_argmax_location_distinguishes_axes():
+    v = np.zeros((6, 5, 4), dtype=np.float32)       # nz=6, ny=5, nx=4
+    v[4, 1, 2] = 7.0                                # z=4, y=1, x=2
+    img = O.render(v, W.ortho_axis_camera((4, 5, 6), 2, +1, step=1.0), O.MIP).image
+    assert img.shape == (5, 4) and img[1, 2] == 7.0 and (img > 0).sum() == 1
+    img = O.render(v, W.ortho_axis_camera((4, 5, 6), 0, +1, step=1.0), O.MIP).image
+    assert img.shape == (6, 5) and img[4, 1] == 7.0 and (img > 0).sum() == 1
+
+
+# --------------------------------------------------------------------------- P2
+@pytest.mark.parametrize("step", [1.0, 0.5, 0.25])
+@pytest.mark.parametrize("prec,tol", [(O.F32, 1e-5), (O.F64, 1e-12)])
+def test_p2_constant_cube_axis_aligned(step, prec, tol):
+    n = (16, 12, 20)
+    v = np.full((20, 12, 16), 0.6, dtype=np.float32)
+    tf = ramp_alpha_tf(0.5)
+    vmin, vmax = 0.0, 1.0
+    u = float(np.float32(0.6))                      # the stored voxel value
+    a, rgb = 0.5 * KS * u, np.array([KS * u, 1 - KS * u, 0.25])
+    for axis in range(3):
+        cam = W.ortho_axis_camera(n, axis, +1, step=step)
+        r = O.render(v, cam, O.EA, tf, vmin, vmax, precision=prec)
+        K = int(round(n[axis] / step))
+        assert np.all(r.K == K)
+        A = 1 - (1 - a) ** K
+        assert np.max(np.abs(r.image64[..., 3] - A)) <= tol
+        assert np.max(np.abs(r.image64[..., :3] - rgb * A)) <= 2 * tol
+
+
+def test_p2_constant_cube_oblique_rays_chord_count():
+    n = (24, 20, 28)
+    v = np.full((28, 20, 24), 0.3, dtype=np.float32)
+    a = 1.0 / 64.0                                  # dyadic: exact in the float32 table
+    tf = const_tf([0.25, 0.5, 0.875, a])
+    cam = W.perspective_camera((60.0, 45.0, -40.0), (12, 10, 14), (0, 1, 0), 30.0, 40, 30, step=0.5)
+    r = O.render(v, cam, O.EA, tf, 0.0, 1.0, precision=O.F64)
+    vec = cam.vectors().astype(np.float64)
+    i, j = np.meshgrid(np.arange(40) + 0.5, np.arange(30) + 0.5)
+    g = vec[3] + i[..., None] * vec[4] + j[..., None] * vec[5]
+    d = g / np.linalg.norm(g, axis=-1, keepdims=True)
+    o = vec[0]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        t0 = (0 - o) / d
+        t1 = (np.array(n) - o) / d
+    te = np.maximum(np.minimum(t0, t1).max(-1), 0.0)
+    tx = np.maximum(t0, t1).min(-1)
+    hit = tx > te
+    L = np.where(hit, tx - te, 0.0)
+    Kcf = np.where(hit, np.ceil(L / 0.5 - 0.5), 0)
+    assert hit.sum() > 200
+    assert np.all(np.abs(r.K - Kcf) <= 1)
+    assert (r.K == Kcf).mean() > 0.98
+    A = 1 - (1 - a) ** r.K
+    assert np.max(np.abs(r.image64[..., 3] - A)) < 1e-12
+    assert np.max(np.abs(r.image64[..., 0] - 0.25 * A)) < 1e-12
+    assert np.all(r.image64[~hit] == 0)
+    r32 = O.render(v, cam, O.EA, tf, 0.0, 1.0)
+    assert np.max(np.abs(r32.image - r.image64)) < 1e-5
+
+
+# --------------------------------------------------------------------------- P3
+def _cams_for_bricks(n):
+    c = np.array(n) / 2
+    yield W.perspective_camera(c + np.array([90.0, 40.0, 70.0]), c, (0, 1, 0), 40.0, 48, 36, step=0.5)
+    yield W.ortho_lookat_camera(c + np.array([-80.0, 30.0, 55.0]), c, (0, 1, 0), 90.0, 40, 30, step=0.7)
+    # adversarial: eye inside the volume, within half a voxel of a brick plane
+    yield W.perspective_camera((16.3, 7.25, 32.45), (30, 40, 10), (0, 0, 1), 70.0, 40, 30, step=0.5)
+    yield W.perspective_camera((15.6, 14.01, 16.49), (0, 50, 70), (0, 1, 0), 80.0, 40, 30, step=0.35)
+
+
+@pytest.mark.parametrize("B", [2, 7, 16, 72, 100])
+def test_p3_bricked_equals_unbricked(B):
+    n = (40, 56, 72)
+    v = noise_cube(*n, seed=3)
+    tf = W.bake_tf(W.TF_HAZE_POINTS, 0.5, alpha_scale=4.0)
+    s = O.minmax_hist(v)
+    for cam in _cams_for_bricks(n):
+        m0 = O.render(v, cam, O.MIP)
+        m1 = O.render(v, cam, O.MIP, brick=B)
+        assert m1.n_noncontig == 0 and m1.n_order_mismatch == 0
+        assert np.array_equal(m0.image, m1.image)                          # MIP bit-exact
+        e0 = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
+        e1 = O.render(v, cam, O.EA, tf, s.vmin, s.vmax, brick=B)
+        assert e1.n_noncontig == 0 and e1.n_order_mismatch == 0
+        assert np.max(np.abs(e0.image - e1.image)) <= 1e-5
+        d0 = O.render(v, cam, O.EA, tf, s.vmin, s.vmax, precision=O.F64)
+        d1 = O.render(v, cam, O.EA, tf, s.vmin, s.vmax, brick=B, precision=O.F64)
+        assert d1.n_noncontig == 0 and d1.n_order_mismatch == 0
+        assert np.max(np.abs(d0.image64 - d1.image64)) <= 1e-12
+        assert np.array_equal(m0.K, m1.K)
+
+
+def test_p3_wrong_order_would_be_detected():
+    """The fold is order-sensitive: reversing the view must change EA (sanity of the pin)."""
+    n = (40, 56, 72)
+    v = noise_cube(*n, seed=3)
+    tf = W.bake_tf(W.TF_HAZE_POINTS, 0.5, alpha_scale=30.0)
+    s = O.minmax_hist(v)
+    a = O.render(v, W.ortho_axis_camera(n, 2, +1, step=0.5), O.EA, tf, s.vmin, s.vmax, brick=16)
+    b = O.render(v, W.ortho_axis_camera(n, 2, -1, step=0.5), O.EA, tf, s.vmin, s.vmax, brick=16)
+    assert np.max(np.abs(a.image[..., :3] - b.image[..., :3])) > 1e-3
+    assert np.max(np.abs(a.image[..., 3] - b.image[..., 3])) < 1e-5     # opacity is order-free
+
+
+def test_bricked_halo_layout_equals_linear():
+    n = (21, 18, 13)
+    v = noise_cube(*n, seed=5)
+    t = W.retile_halo(v, 8)
+    cam = W.perspective_camera((50.0, 30.0, 40.0), (10, 9, 6), (0, 1, 0), 35.0, 32, 24, step=0.5)
+    a = O.render(v, cam, O.MIP)
+    b = O.render(t, cam, O.MIP, layout=O.BRICKED_HALO1, layout_brick=8, dims=n)
+    assert np.array_equal(a.image, b.image)
+    sa, sb = O.minmax_hist(v), O.minmax_hist(t, layout=O.BRICKED_HALO1, layout_brick=8, dims=n)   # P14
+    assert sa.vmin == sb.vmin and sa.vmax == sb.vmax and np.array_equal(sa.counts, sb.counts)
+    assert sb.counts.sum() == v.size                                        # halo not double counted
+
+
+# --------------------------------------------------------------------------- P4
+def test_p4_minmax_hist_closed_forms():
+    # integers 0..255 uniformly: each of 256 bins holds exactly N/256; v == max lands in the last bin
+    v = (np.arange(8 * 16 * 32) % 256).astype(np.float32).reshape(8, 16, 32)
+    RNG.shuffle(v.reshape(-1))
+    s = O.minmax_hist(v)
+    assert s.vmin == 0 and s.vmax == 255 and np.all(s.counts == v.size // 256)
+    assert s.n_below == s.n_above == s.n_nonfinite == 0
+    # constant cube -> everything in bin 0 (hi == lo)
+    s = O.minmax_hist(np.full((4, 5, 6), 3.5, dtype=np.float32))
+    assert s.vmin == s.vmax == np.float32(3.5) and s.counts[0] == 120 and s.counts[1:].sum() == 0
+    # planted NaN / +-Inf are skipped by min/max and counted
+    v = noise_cube(10, 11, 12).copy()
+    v[0, 0, 0], v[3, 4, 5], v[9, 9, 9], v[5, 5, 5] = np.nan, np.inf, -np.inf, np.nan
+    s = O.minmax_hist(v)
+    fin = v[np.isfinite(v)]
+    assert s.n_nonfinite == 4 and s.vmin == fin.min() and s.vmax == fin.max()
+    assert s.counts.sum() + s.n_below + s.n_above + s.n_nonfinite == v.size
+    assert s.counts[-1] >= 1 and s.counts[0] >= 1
+    # caller range narrower than the data
+    s = O.minmax_hist(v, 16, (-1.0, 1.0))
+    assert s.n_below == (fin < -1).sum() and s.n_above == (fin > 1).sum()
+    assert s.counts.sum() == ((fin >= -1) & (fin <= 1)).sum()
+
+
+def test_p4_histogram_matches_numpy_library_routine():
+    # values at bin centres: no edge ambiguity, must equal np.histogram exactly
+    nb, lo, hi = 64, -2.0, 6.0
+    k = RNG.integers(0, nb, size=5000)
+    v = (lo + (k + 0.5) * (hi - lo) / nb).astype(np.float32).reshape(10, 20, 25)
+    s = O.minmax_hist(v, nb, (lo, hi))
+    want, _ = np.histogram(v.astype(np.float64), bins=nb, range=(lo, hi))
+    assert np.array_equal(s.counts, want.astype(np.uint64))
+    # random data over [min,max]: float32 edge rounding may move a voxel to the adjacent bin only
+    v = noise_cube(40, 30, 20, seed=8)
+    s = O.minmax_hist(v)
+    want, _ = np.histogram(v.astype(np.float64), bins=256, range=(float(s.vmin), float(s.vmax)))
+    diff = s.counts.astype(np.int64) - want
+    assert diff.sum() == 0 and np.abs(diff).sum() <= 8
+    assert np.abs(np.cumsum(diff)).max() <= 2
+
+
+# --------------------------------------------------------------------------- P5 / P7
+def _affine_setup():
+    n = (20, 16, 24)
+    al, be, ga, de = 0.031, -0.017, 0.023, 0.4
+    z, y, x = np.meshgrid(np.arange(24), np.arange(16), np.arange(20), indexing="ij")
+    v = (al * x + be * y + ga * z + de).astype(np.float32)
+    cam = W.perspective_camera((55.0, 38.0, -30.0), (10, 8, 12), (0, 1, 0), 32.0, 36, 28, step=0.5)
+    return n, (al, be, ga, de), v, cam
+
+
+def _closed_form_samples(n, coef, cam, K):
+    """Double-precision sample positions (C.1-C.2) and the affine value at each (clamp-to-edge)."""
+    al, be, ga, de = coef
+    vec = cam.vectors().astype(np.float64)
+    out = {}
+    for j in range(cam.height):
+        for i in range(cam.width):
+            if K[j, i] == 0:
+                continue
+            g = vec[3] + (i + 0.5) * vec[4] + (j + 0.5) * vec[5]
+            d = g / np.linalg.norm(g)
+            o = vec[0] + (i + 0.5) * vec[1] + (j + 0.5) * vec[2]
+            with np.errstate(divide="ignore"):
+                t0, t1 = (0 - o) / d, (np.array(n) - o) / d
+            te = max(0.0, np.minimum(t0, t1).max())
+            tx = np.maximum(t0, t1).min()
+            t = te + (np.arange(K[j, i]) + 0.5) * cam.step
+            if not (t[-1] < tx - 1e-6 and te + (K[j, i] + 0.5) * cam.step > tx + 1e-6):
+                continue                                    # K ambiguous at the exit face: skip
+            p = o + t[:, None] * d - 0.5
+            p = np.clip(p, 0, np.array(n) - 1.0)
+            out[(j, i)] = al * p[:, 0] + be * p[:, 1] + ga * p[:, 2] + de
+    return out
+
+
+def test_p5_affine_cube_mip_and_ea_closed_sum():
+    n, coef, v, cam = _affine_setup()
+    tf = ramp_alpha_tf(0.125)
+    vmin, vmax = 0.0, 2.0
+    m32, m64 = O.render(v, cam, O.MIP), O.render(v, cam, O.MIP, precision=O.F64)
+    e32 = O.render(v, cam, O.EA, tf, vmin, vmax)
+    e64 = O.render(v, cam, O.EA, tf, vmin, vmax, precision=O.F64)
+    S = _closed_form_samples(n, coef, cam, m64.K)
+    assert len(S) > 150
+    for (j, i), s in S.items():
+        mx = s.max()
+        assert abs(m64.image64[j, i] - mx) < 5e-7        # float32 voxels of an affine field: ~6e-8 each
+        assert abs(m32.image[j, i] - mx) < 2e-5
+        u = np.clip((s - vmin) / (vmax - vmin), 0, 1)
+        a = 0.125 * KS * u
+        Tk = np.concatenate([[1.0], np.cumprod(1 - a)])[:-1]
+        w = Tk * a
+        want = np.array([(w * KS * u).sum(), (w * (1 - KS * u)).sum(), (w * 0.25).sum(), 1 - np.prod(1 - a)])
+        assert np.max(np.abs(e64.image64[j, i] - want)) < 2e-6
+        assert np.max(np.abs(e32.image[j, i] - want)) < 2e-5
+
+
+def test_p7_alpha_zero_and_alpha_one():
+    n, coef, v, cam = _affine_setup()
+    r = O.render(v, cam, O.EA, const_tf([0.3, 0.6, 0.9, 0.0]), 0.0, 2.0)
+    assert np.all(r.image == 0)
+    w = np.arange(256, dtype=np.float64) / 256.0
+    tf = np.stack([w, 1 - w, 0.5 * w, np.ones_like(w)], axis=1).astype(np.float32)
+    r = O.render(v, cam.with_(ert_alpha=0.99), O.EA, tf, 0.0, 2.0, precision=O.F64)
+    S = _closed_form_samples(n, coef, cam, r.K)
+    hit = r.K > 0
+    assert np.all(r.K_ert[hit] == 1) and np.all(r.image64[hit][:, 3] == 1.0)
+    for (j, i), s in S.items():
+        u0 = KS * s[0] / 2.0
+        assert np.max(np.abs(r.image64[j, i, :3] - [u0, 1 - u0, 0.5 * u0])) < 1e-6
+    r0 = O.render(v, cam, O.EA, tf, 0.0, 2.0, precision=O.F64)               # ERT off: same image, all K
+    assert np.array_equal(r0.image64, r.image64) and np.array_equal(r0.K_ert, r0.K)
+
+
+# --------------------------------------------------------------------------- P6
+def test_p6_impulse_tent_footprint():
+    n = (9, 8, 7)
+    v = np.zeros((7, 8, 9), dtype=np.float32)
+    x0, y0, z0, amp = 4, 3, 2, 8.0
+    v[z0, y0, x0] = amp
+    W_, H_ = 9 * 4, 8 * 4
+    cam = W.ortho_axis_camera(n, 2, +1, step=0.25, width=W_, height=H_)
+    r = O.render(v, cam, O.MIP)
+    xs = (np.arange(W_) + 0.5) * 9 / W_
+    ys = (np.arange(H_) + 0.5) * 8 / H_
+    wx = np.maximum(0, 1 - np.abs(xs - (x0 + 0.5)))
+    wy = np.maximum(0, 1 - np.abs(ys - (y0 + 0.5)))
+    want = amp * wy[:, None] * wx[None, :] * 0.875          # nearest sample is 1/8 voxel from the centre plane
+    assert np.max(np.abs(r.image - want)) < 1e-6
+    # boundary voxel: clamp-to-edge extends the value constantly through the outer half voxel
+    v[:] = 0
+    v[3, 0, 0] = amp
+    r = O.render(v, W.ortho_axis_camera(n, 2, +1, step=0.25, width=W_, height=H_), O.MIP)
+    wx = np.where(xs <= 0.5, 1.0, np.maximum(0, 1 - np.abs(xs - 0.5)))
+    wy = np.where(ys <= 0.5, 1.0, np.maximum(0, 1 - np.abs(ys - 0.5)))
+    assert np.max(np.abs(r.image - amp * wy[:, None] * wx[None, :] * 0.875)) < 1e-6
+
+
+# --------------------------------------------------------------------------- P8
+@pytest.mark.parametrize("step", [1.0, 0.5, 0.25])
+def test_p8_sample_counts(step):
+    n = (10, 12, 14)
+    v = noise_cube(*n)
+    for axis in range(3):
+        cam = W.ortho_axis_camera(n, axis, -1, step=step)
+        r = O.render(v, cam, O.MIP)
+        assert r.n_nominal == cam.width * cam.height * int(n[axis] / step)
+        assert r.n_ert == r.n_nominal
+
+
+def test_misses_and_degenerate_rays():
+    n = (10, 12, 14)
+    v = noise_cube(*n)
+    cam = W.perspective_camera((100.0, 100.0, 100.0), (200, 200, 200), (0, 1, 0), 20.0, 16, 12)   # looks away
+    r = O.render(v, cam, O.MIP)
+    assert np.all(np.isneginf(r.image)) and r.n_nominal == 0
+    r = O.render(v, cam, O.EA, const_tf([1, 1, 1, 0.5]), 0.0, 1.0)
+    assert np.all(r.image == 0)
+    # d_a == 0 with the origin outside that slab: miss (S6), inside: hit
+    cam = W.ortho_axis_camera(n, 2, +1, step=1.0, width=20, height=12)
+    cam = cam.with_(ou=np.array([1.0, 0, 0], dtype=np.float32), o0=np.array([-5.0, 0, -1], dtype=np.float32))
+    r = O.render(v, cam, O.MIP)
+    assert np.all(np.isneginf(r.image[:, :5])) and np.all(np.isfinite(r.image[:, 5:15])) and np.all(np.isneginf(r.image[:, 15:]))
+
+
+# --------------------------------------------------------------------------- P9
+def test_p9_mirror_symmetry():
+    n = (24, 18, 20)
+    v = noise_cube(*n, seed=2)
+    tf = W.bake_tf(W.TF_HAZE_POINTS, 0.5, alpha_scale=8.0)
+    s = O.minmax_hist(v)
+    cam = W.perspective_camera((70.0, 41.0, -33.0), (12, 9, 10), (0, 1, 0), 30.0, 40, 30, step=0.5)
+    vec = cam.vectors().copy()
+    mir = vec.copy()
+    mir[:, 0] *= -1
+    mir[0, 0] = 24.0 - vec[0, 0]
+    camm = cam.with_(o0=mir[0], ou=mir[1], ov=mir[2], d0=mir[3], du=mir[4], dv=mir[5])
+    vm = np.ascontiguousarray(v[:, :, ::-1])
+    for mode, kw in ((O.MIP, {}), (O.EA, dict(tf=tf, vmin=s.vmin, vmax=s.vmax))):
+        a = O.render(v, cam, mode, precision=O.F64, **kw)
+        b = O.render(vm, camm, mode, precision=O.F64, **kw)
+        assert np.array_equal(a.K, b.K)
+        fin = np.isfinite(a.image64)
+        assert np.array_equal(fin, np.isfinite(b.image64))
+        assert np.max(np.abs(a.image64[fin] - b.image64[fin])) < 1e-9
+        a = O.render(v, cam, mode, **kw)
+        b = O.render(vm, camm, mode, **kw)
+        fin = np.isfinite(a.image)
+        assert np.max(np.abs(a.image[fin] - b.image[fin])) < 2e-4
+
+
+# --------------------------------------------------------------------------- P11
+def test_p11_ert_bound_and_fragility():
+    n = (40, 40, 48)
+    v = W.make_cube(W.Recipe(*n, seed=4, n_sources=6))
+    s = O.minmax_hist(v)
+    tf = W.bake_tf(W.TF_HAZE_POINTS, 0.5, alpha_scale=40.0)
+    cam = W.perspective_camera((110.0, 60.0, 95.0), (20, 20, 24), (0, 1, 0), 30.0, 64, 48, step=0.5)
+    full = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
+    ert = O.render(v, cam.with_(ert_alpha=0.99), O.EA, tf, s.vmin, s.vmax)
+    assert ert.n_ert < full.n_ert and ert.n_nominal == full.n_nominal
+    assert (ert.K_ert < ert.K).sum() > 50                       # ERT actually fires
+    assert np.all(ert.image <= full.image + 1e-6)
+    assert np.max(full.image - ert.image) <= (1 - 0.99) + 1e-4
+    stopped = ert.K_ert < ert.K
+    assert np.all(ert.image[stopped][:, 3] >= 0.99 - 1e-6)
+    assert ert.fragile.mean() < 0.005
+    # bricked request with ERT on renders by the single march (C.7 / S15)
+    eb = O.render(v, cam.with_(ert_alpha=0.99), O.EA, tf, s.vmin, s.vmax, brick=16)
+    assert np.array_equal(eb.image, ert.image)
+
+
+# --------------------------------------------------------------------------- P12 / P13
+def test_p12_f32_canonical_close_to_f64_truth():
+    n = (96, 96, 96)
+    v = noise_cube(*n, seed=6)
+    cam = W.orbit_camera(n, 1, 8, 96, 96, step=0.5)
+    a = O.render(v, cam, O.MIP)
+    b = O.render(v, cam, O.MIP, precision=O.F64)
+    hit = np.isfinite(b.image64)
+    assert np.array_equal(hit, np.isfinite(a.image))
+    R = float(np.abs(v).max())
+    rel = np.abs(a.image[hit] - b.image64[hit]) / np.maximum(np.abs(b.image64[hit]), R)
+    assert np.median(rel) < 1e-5 and rel.max() < 1e-3
+
+
+def test_p13_step_halving_converges_on_smooth_cube():
+    n = (48, 48, 48)
+    v = W.make_cube(W.Recipe(*n, seed=10, n_sources=5, noise_amp=0.0))
+    cam0 = W.perspective_camera((130.0, 70.0, 110.0), (24, 24, 24), (0, 1, 0), 28.0, 40, 40)
+    imgs = []
+    for step in (1.0, 0.5, 0.25, 0.125):
+        tf = W.bake_tf(W.TF_HAZE_POINTS, step, alpha_scale=3.0)
+        imgs.append(O.render(v, cam0.with_(step=step), O.EA, tf, 0.0, float(v.max()), precision=O.F64).image64)
+    e = [np.abs(imgs[k] - imgs[k + 1]).max() for k in range(3)]
+    assert e[0] > e[1] > e[2] and e[2] < 0.35 * e[0]

@@ -1,0 +1,42 @@
+"""Transfer-function tables (input generation, readings S11/S31).
+
+A table is 256 x RGBA float32, entry i at u = i/255, rgb non-premultiplied, alpha = the
+per-SAMPLE opacity at the render's step.  Opacity correction alpha_step = 1-(1-alpha_1)^step
+is baked HERE in double; the library and the oracle apply no correction of their own.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+# (u, r, g, b, alpha per unit voxel length)
+TF_HAZE_POINTS = (
+    (0.00, 0.0, 0.0, 0.0, 0.0),
+    (0.15, 0.0, 0.0, 0.2, 0.0),
+    (0.30, 0.0, 0.3, 0.8, 0.004),
+    (0.50, 0.9, 0.8, 0.1, 0.08),
+    (1.00, 1.0, 1.0, 1.0, 0.6),
+)
+
+
+def bake_tf(points, step: float, alpha_scale: float = 1.0, alpha_clip: float = 1.0) -> np.ndarray:
+    """Piecewise-linear control points -> (256,4) float32 table with step-baked alpha."""
+    p = np.asarray(points, dtype=np.float64)
+    u = np.arange(256, dtype=np.float64) / 255.0
+    tab = np.stack([np.interp(u, p[:, 0], p[:, c]) for c in range(1, 5)], axis=1)
+    a1 = np.clip(tab[:, 3] * alpha_scale, 0.0, alpha_clip)
+    tab[:, 3] = 1.0 - np.power(1.0 - a1, step)
+    return np.clip(tab, 0.0, 1.0).astype(np.float32)
+
+
+def kappa(dims) -> float:
+    return 256.0 / float(max(dims))
+
+
+def tf_haze(dims, step: float) -> np.ndarray:
+    """TF_HAZE: noise faintly emissive, no empty-space shortcut, ERT fires only behind sources."""
+    return bake_tf(TF_HAZE_POINTS, step, alpha_scale=kappa(dims))
+
+
+def tf_opaque(dims, step: float) -> np.ndarray:
+    """TF_OPAQUE: TF_HAZE with alpha x25 clamped to 1 (ERT parity workload; ERT-assisted timing)."""
+    return bake_tf(TF_HAZE_POINTS, step, alpha_scale=25.0 * kappa(dims))
