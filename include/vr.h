@@ -1,0 +1,227 @@
+/*
+ * vr.h — C ABI of libvr.so: B200-native bricked volume ray-casting of float32 spectral
+ * cubes plus the min/max + histogram summary passes.
+ *
+ * What is computed.  The paper names the operations — interactive volume rendering of
+ * larger-than-memory spectral cubes by sub-cube partitioning and a gather of partial images
+ * and the "simple data analysis tasks" minimum/maximum
+ * and histogram — but gives no formulae.  The arithmetic is therefore the
+ * set of readings C.0-C.8 of SURVEY.md §8(c), restated in DESIGN.md §3.  Every entry point
+ * below cites the passage and the reading it implements.
+ *
+ * Conventions common to all calls
+ *   - Plain C, no CUDA or torch types: a stream is passed as `void*` holding a cudaStream_t
+ *     (NULL = the legacy default stream).  Pointers are marked HOST or DEVICE.
+ *   - Every call returns vr_status; nothing throws, aborts or prints.  vr_last_error() gives a
+ *     thread-local message for the last failing call on this thread.
+ *   - Every struct starts with `struct_size` = sizeof(that struct) as the caller compiled it.
+ *   - vr_render / vr_minmax_histogram ENQUEUE work on `stream` and return; results are valid
+ *     once `stream` reaches the point after the call.  With device-resident volumes and
+ *     device outputs there is no host synchronisation inside.  Library-internal copy streams
+ *     are joined to `stream` by events.
+ *   - One host thread per handle at a time.  Different handles may be used concurrently.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with VR_ERR_CUDA.
+ */
+#ifndef VR_H_
+#define VR_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define VR_API __attribute__((visibility("default")))
+#else
+#define VR_API
+#endif
+
+typedef enum {
+    VR_OK = 0,
+    VR_ERR_INVALID_ARG = 1,   /* NULL, bad size/enum, non-finite or out-of-range value */
+    VR_ERR_UNSUPPORTED = 2,   /* valid request this build cannot serve (message says why) */
+    VR_ERR_OUT_OF_MEMORY = 3, /* host or device allocation failed */
+    VR_ERR_CUDA = 4,          /* CUDA runtime error (message carries cudaGetErrorString) */
+    VR_ERR_NOT_READY = 5      /* e.g. EA render before vr_set_transfer_function */
+} vr_status;
+
+enum { VR_LINEAR = 0,          /* float32[nz][ny][nx], x fastest (FITS order; z = spectral axis) */
+       VR_BRICKED_HALO1 = 1 }; /* brick-major: brick id = bx + nbx*(by + nby*bz); each brick is
+                                  float32[B+1][B+1][B+1] holding voxels [B*b, B*b+B] per axis clamped
+                                  to the volume (one-voxel high-side halo, C.7) */
+enum { VR_DEVICE = 0, VR_HOST_PINNED = 1 };
+enum { VR_EA = 0,              /* emission-absorption, premultiplied RGBA, 4 channels */
+       VR_MIP = 1 };           /* maximum intensity projection, 1 channel */
+enum { VR_SORT_LAST = 1u };    /* vr_camera.flags: render per-brick partial images and merge them
+                                  with the sort-last compositor even when a single march would do */
+
+typedef struct vr_volume vr_volume; /* opaque; created and destroyed only by the library */
+
+/* ------------------------------------------------------------------------------------------
+ * vr_create_volume — brick decomposition + residency (
+ * PAPER.md:L24, L66 "partitioning the cube into ... sub-cubes, with a different data loading
+ * for each"; reading C.7 for the brick grid).
+ *
+ *   nx,ny,nz   voxels per axis, each >= 2.
+ *   brick      brick edge B in voxels; 0 = one brick = the whole cube.  The grid is
+ *              nb_a = ceil(n_a / B); at most 65535 bricks per axis.
+ *   layout     VR_LINEAR or VR_BRICKED_HALO1 (requires brick > 0).
+ *   location   VR_DEVICE: `data` is a DEVICE pointer, 16-byte aligned, used in place.
+ *              VR_HOST_PINNED: `data` is a HOST pointer to page-locked memory (checked with
+ *              cudaPointerGetAttributes; pageable memory => VR_ERR_INVALID_ARG).  The library
+ *              then owns a device-side copy policy:
+ *                - resident_bytes == 0 or >= the volume's bytes: the whole volume is mirrored
+ *                  on the device on first use (uploaded once on the copy streams);
+ *                - otherwise (out of core; "multiple execution
+ *                  queues (or streams) to overlap GPU computation with data I/O"): a pool of
+ *                  floor(resident_bytes / brick_bytes) brick slots; bricks are streamed per
+ *                  frame in view order on n_copy_streams streams.  Requires VR_BRICKED_HALO1.
+ *   data       BORROWED until vr_destroy_volume; never written by the library.
+ *   n_copy_streams  1..8 (0 => 4).  Only used for VR_HOST_PINNED.
+ * Errors: VR_ERR_INVALID_ARG (NULL, dims < 2, bad enums, brick grid too large, pageable host
+ * memory, misaligned device pointer), VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+    uint32_t struct_size;
+    uint32_t nx, ny, nz;
+    uint32_t brick;
+    uint32_t layout;
+    uint32_t location;
+    uint32_t n_copy_streams;
+    const float *data;          /* DEVICE or pinned HOST, see location */
+    uint64_t resident_bytes;
+} vr_volume_desc;
+
+VR_API vr_status vr_create_volume(const vr_volume_desc *desc, vr_volume **out);
+
+/* Synchronises the library's own streams, frees everything the handle owns.  The caller's
+ * data, image and summary buffers are untouched.  NULL is accepted. */
+VR_API vr_status vr_destroy_volume(vr_volume *vol);
+
+/* ------------------------------------------------------------------------------------------
+ * vr_set_transfer_function — SURVEY.md row A3; reading C.4 (S8-S11).
+ *   rgba   HOST, 256*4 floats, copied before return.  Entry i sits at u = i/255; rgb is
+ *          non-premultiplied; alpha is the per-SAMPLE opacity at the step the caller will
+ *          render with (no opacity correction inside the library).  Every value must be
+ *          finite and in [0,1].
+ *   vmin,vmax  scalar range mapped to u in [0,1]: scale = 1/(vmax-vmin), bias = -vmin*scale,
+ *          both rounded to float32 once (C.4).  Must be finite with vmax > vmin.  Normally
+ *          the vmin/vmax produced by vr_minmax_histogram.
+ * The table is uploaded with a synchronous copy; safe to call between frames.
+ * Errors: VR_ERR_INVALID_ARG, VR_ERR_CUDA.
+ * ------------------------------------------------------------------------------------------ */
+VR_API vr_status vr_set_transfer_function(vr_volume *vol, const float *rgba, float vmin, float vmax);
+
+/* ------------------------------------------------------------------------------------------
+ * vr_render — SURVEY.md rows A4-A10: per-frame brick ordering, ray generation and entry/exit
+ * (C.1, C.2), trilinear sampling (C.3), classification (C.4), front-to-back compositing with
+ * early ray termination (C.5), MIP (C.6), per-brick partial images and the sort-last
+ * compositor (C.7).  This is the kernel the paper calls "the GPU part" of its case study
+ * and the gather of partial results.
+ *
+ * Camera (C.1):  origin(i,j) = o0 + (i+.5)*ou + (j+.5)*ov
+ *                dir(i,j)    = normalize(d0 + (i+.5)*du + (j+.5)*dv)
+ *   in voxel units of the box [0,nx]x[0,ny]x[0,nz]; voxel (ix,iy,iz) has its value at its
+ *   centre (ix+.5, iy+.5, iz+.5); reconstruction is clamp-to-edge (C.0).  Perspective:
+ *   ou = ov = 0.  Orthographic: du = dv = 0.
+ *   step       sample spacing in voxels along the unit direction, > 0.  Samples sit on one
+ *              lattice per ray anchored at the VOLUME entry: t_k = t_enter + (k+.5)*step.
+ *   ert_alpha  0 = off; otherwise in (0,1): a ray stops after the sample at which its
+ *              transmittance T <= 1 - ert_alpha (that sample included).  EA only.
+ *   flags      VR_SORT_LAST: per-brick partial images + compositor.  Needs brick > 0, a pure
+ *              perspective or pure orthographic camera, and ert_alpha == 0 (early termination
+ *              is not defined for independent partials, reading S15) => else VR_ERR_UNSUPPORTED.
+ * Image: `pixels` is caller-owned, DEVICE (location VR_DEVICE) or pinned HOST (VR_HOST_PINNED;
+ *   the library renders into an internal device image and enqueues the device-to-host copy on
+ *   `stream`).  Row j = 0 is the v-minimum row; row_pitch_bytes >= width*channels*4 and a
+ *   multiple of 16 (EA) / 4 (MIP); 0 means tightly packed.
+ *   VR_EA : channels = 4: premultiplied (C.r, C.g, C.b, 1-T); a miss is (0,0,0,0).
+ *   VR_MIP: channels = 1: max of the interpolated samples in data units; no sample = -INFINITY.
+ * Out-of-core volumes are rendered brick by brick in view order with the ray state carried in
+ * the image (so ERT stays exact); uploads run on the copy streams and overlap rendering.
+ * Errors: VR_ERR_INVALID_ARG (NULL, width/height 0, step <= 0 or non-finite, ert_alpha not in
+ * [0,1), channels not matching mode, bad pitch), VR_ERR_NOT_READY (EA before a transfer
+ * function was set), VR_ERR_UNSUPPORTED, VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+    uint32_t struct_size, width, height;
+    float o0[3], ou[3], ov[3];
+    float d0[3], du[3], dv[3];
+    float step;
+    float ert_alpha;
+    uint32_t flags;
+} vr_camera;
+
+typedef struct {
+    uint32_t struct_size;
+    uint32_t channels;          /* 4 for VR_EA, 1 for VR_MIP */
+    uint32_t location;          /* VR_DEVICE or VR_HOST_PINNED */
+    uint32_t reserved;
+    float *pixels;
+    uint64_t row_pitch_bytes;
+} vr_image;
+
+VR_API vr_status vr_render(vr_volume *vol, const vr_camera *cam, int mode, const vr_image *image, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * vr_minmax_histogram — SURVEY.md rows A1, A2; reading C.8 (S22-S26).
+ * ("calculating a histogram or computing data minimum/maximum"), L66 ("a single-pass
+ * accumulative operation like calculating the data minimum and maximum").
+ *
+ *   vmin, vmax   min and max over the voxels with isfinite(v); n_nonfinite counts the rest.
+ *   histogram    lo,hi = range[0],range[1] if range != NULL else (vmin,vmax);
+ *                scale_h = (float)nbins / (hi - lo)  (0 if hi == lo); for each finite v:
+ *                v < lo => n_below; v > hi => n_above; else b = (int)((v - lo) * scale_h),
+ *                clamped to nbins-1; counts[b]++.  All float32, subtract then multiply, no FMA.
+ *                Invariant: sum(counts) + n_below + n_above + n_nonfinite == nx*ny*nz.
+ *                Halo voxels of a bricked layout are not counted.
+ *   nbins        1..4096.
+ *   range        HOST pointer to two floats (finite, range[1] >= range[0]) or NULL.  With NULL
+ *                the cube is read twice (8 B/voxel), else once for min/max and histogram together.
+ *   out          vr_summary followed by nbins uint64 counts: DEVICE memory (out_location
+ *                VR_DEVICE) or pinned HOST (VR_HOST_PINNED), 8-byte aligned,
+ *                VR_SUMMARY_BYTES(nbins) bytes, written on `stream`.
+ * Out-of-core volumes are streamed through the brick pool (both passes ride the streamer).
+ * Errors: VR_ERR_INVALID_ARG, VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+    float vmin, vmax;
+    uint64_t n_nonfinite, n_below, n_above;
+    uint64_t counts[1];         /* nbins entries */
+} vr_summary;
+#define VR_SUMMARY_BYTES(nbins) (32u + 8u * (uint64_t)(nbins))
+
+VR_API vr_status vr_minmax_histogram(vr_volume *vol, uint32_t nbins, const float *range, vr_summary *out,
+                                     uint32_t out_location, void *stream);
+
+/* ------------------------------------------------------------------------------------------
+ * vr_get_stats — counters of the last vr_render / vr_minmax_histogram on this handle
+ * (SURVEY.md §5 "metrics"): host-side values only, no synchronisation.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+    uint32_t struct_size;
+    uint32_t n_bricks;              /* bricks in the grid */
+    uint32_t bricks_drawn;          /* bricks that produced work in the last render */
+    uint32_t bricks_culled;         /* bricks outside the view (empty screen rectangle) */
+    uint32_t path;                  /* last render: 0 none, 1 single march, 2 sort-last, 3 streamed chain */
+    uint32_t kernel_launches;       /* library kernels launched by the last call */
+    uint64_t fragments;             /* (brick,pixel) partial fragments written (sort-last) */
+    uint64_t h2d_bytes;             /* host-to-device bytes enqueued by the last call */
+    uint64_t d2h_bytes;             /* device-to-host bytes enqueued by the last call */
+    uint64_t total_kernel_launches; /* since vr_create_volume */
+    uint64_t resident_bytes;        /* device bytes owned by the handle */
+} vr_stats;
+
+VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
+
+/* Thread-local message of the last failing call on this thread ("" if none). */
+VR_API const char *vr_last_error(void);
+
+/* Library version and the CUDA architecture it was built for, e.g. "vr-b200 0.1 sm_100a". */
+VR_API const char *vr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VR_H_ */

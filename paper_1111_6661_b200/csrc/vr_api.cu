@@ -1,0 +1,714 @@
+// vr_api.cu — the C ABI of include/vr.h and the host runtime behind it: brick table and
+// residency, per-frame brick ordering / culling / screen rectangles (A4),
+// the out-of-core brick streamer (A5) and launch planning for the kernels of vr_raycast.cu and
+// vr_reduce.cu.  No host synchronisation on the in-HBM paths; everything is enqueued on the
+// caller's stream, library copy streams are joined to it by events.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "vr_internal.h"
+
+namespace vr {
+
+// ------------------------------------------------------------------ error plumbing
+static thread_local char g_err[512] = "";
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+vr_status cuda_fail(cudaError_t e, const char *what)
+{
+    set_error("CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return VR_ERR_OUT_OF_MEMORY; }
+    return VR_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------ small helpers
+template <typename T>
+struct DevBuf {                       // grow-only device buffer
+    T *p = nullptr;
+    size_t cap = 0;
+    vr_status reserve(size_t n)
+    {
+        if (n <= cap) return VR_OK;
+        if (p) { VR_CUDA(cudaFree(p)); p = nullptr; cap = 0; }
+        size_t want = n + n / 4;
+        VR_CUDA(cudaMalloc(&p, want * sizeof(T)));
+        cap = want;
+        return VR_OK;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
+struct Staging {                      // one slot of the per-frame table ring (pinned host + device)
+    unsigned char *h = nullptr, *d = nullptr;
+    size_t cap = 0;
+    cudaEvent_t done = nullptr;       // recorded after the last kernel that reads d
+    bool in_flight = false;
+};
+
+constexpr int kStagingRing = 4;
+constexpr int kMaxCopyStreams = 8;
+
+}  // namespace vr
+
+using namespace vr;
+
+struct vr_volume {
+    vr_volume_desc desc;
+    int device = 0, sm_count = 0;
+    uint32_t B = 0, E = 0;                    // brick edge; E = B + 1 (bricked layouts)
+    uint32_t nb[3] = { 1, 1, 1 };
+    uint64_t n_vox = 0, n_bricks = 1, brick_elems = 0, total_elems = 0;
+    bool out_of_core = false;
+
+    // device views
+    const float *dev_data = nullptr;          // whole volume on the device in desc.layout (borrowed or mirror)
+    float *mirror = nullptr;                  // owned copy of a host volume (fully resident case)
+    bool mirror_valid = false;
+    std::vector<cudaEvent_t> mirror_ev;       // one per copy stream used by the upload
+
+    // out-of-core pool
+    float *pool = nullptr;
+    uint32_t n_slots = 0, n_fixed = 0, n_ring = 0;
+    uint64_t ring_pos = 0, copy_rr = 0;
+    std::vector<uint8_t> fixed_loaded;
+    std::vector<cudaEvent_t> ev_up, ev_free;  // per slot
+    std::vector<uint8_t> slot_used;
+
+    cudaStream_t copy[kMaxCopyStreams] = {};
+    int n_copy = 0;
+
+    // transfer function
+    float4 *d_tf = nullptr;
+    bool tf_set = false;
+    float tf_scale = 0.0f, tf_bias = 0.0f;
+
+    // scratch
+    SummaryScratch *d_sum = nullptr;
+    vr_summary *d_sum_out = nullptr;          // staging for host outputs
+    DevBuf<float> arena, host_image;
+    Staging staging[kStagingRing];
+    int staging_next = 0;
+
+    vr_stats stats;
+};
+
+namespace vr {
+
+static void free_volume(vr_volume *v)
+{
+    if (!v) return;
+    cudaSetDevice(v->device);
+    for (int i = 0; i < v->n_copy; ++i) if (v->copy[i]) { cudaStreamSynchronize(v->copy[i]); cudaStreamDestroy(v->copy[i]); }
+    for (auto e : v->mirror_ev) cudaEventDestroy(e);
+    for (auto e : v->ev_up) cudaEventDestroy(e);
+    for (auto e : v->ev_free) cudaEventDestroy(e);
+    for (auto &s : v->staging) {
+        if (s.done) { if (s.in_flight) cudaEventSynchronize(s.done); cudaEventDestroy(s.done); }
+        if (s.h) cudaFreeHost(s.h);
+        if (s.d) cudaFree(s.d);
+    }
+    if (v->mirror) cudaFree(v->mirror);
+    if (v->pool) cudaFree(v->pool);
+    if (v->d_tf) cudaFree(v->d_tf);
+    if (v->d_sum) cudaFree(v->d_sum);
+    if (v->d_sum_out) cudaFree(v->d_sum_out);
+    v->arena.release();
+    v->host_image.release();
+    delete v;
+}
+
+static inline uint64_t brick_id(const vr_volume *v, uint32_t bx, uint32_t by, uint32_t bz)
+{
+    return bx + (uint64_t)v->nb[0] * (by + (uint64_t)v->nb[1] * bz);
+}
+
+// owned base-index range of brick b on axis a (C.7): i0 in [B*b, min(B*b + B - 1, n - 2)]
+static inline void owned_range(const vr_volume *v, int a, uint32_t b, int &lo, int &hi)
+{
+    const int n = (int)(a == 0 ? v->desc.nx : a == 1 ? v->desc.ny : v->desc.nz);
+    lo = (int)(v->B * b);
+    hi = std::min((int)(v->B * b + v->B - 1), n - 2);
+}
+
+// make sure a fully-resident host volume is on the device; `st` then waits for the upload
+static vr_status ensure_mirror(vr_volume *v, cudaStream_t st)
+{
+    if (v->desc.location != VR_HOST_PINNED || v->out_of_core) return VR_OK;
+    if (!v->mirror_valid) {
+        const size_t bytes = v->total_elems * sizeof(float);
+        const size_t chunk = std::max<size_t>((bytes / (size_t)v->n_copy + 255) & ~(size_t)255, 256);
+        size_t off = 0;
+        for (int i = 0; i < v->n_copy && off < bytes; ++i, off += chunk) {
+            const size_t nby = std::min(chunk, bytes - off);
+            VR_CUDA(cudaMemcpyAsync((char *)v->mirror + off, (const char *)v->desc.data + off, nby,
+                                    cudaMemcpyHostToDevice, v->copy[i]));
+            VR_CUDA(cudaEventRecord(v->mirror_ev[i], v->copy[i]));
+        }
+        v->mirror_valid = true;
+        v->stats.h2d_bytes += bytes;
+    }
+    for (auto e : v->mirror_ev) VR_CUDA(cudaStreamWaitEvent(st, e, 0));
+    return VR_OK;
+}
+
+// device pointer + strides + origin of brick (bx,by,bz) for the resident layouts
+static void resident_brick_view(const vr_volume *v, uint32_t bx, uint32_t by, uint32_t bz, BrickK &k)
+{
+    if (v->desc.layout == VR_LINEAR) {
+        k.base = v->dev_data; k.sy = v->desc.nx; k.sz = (long long)v->desc.nx * v->desc.ny;
+        k.ox = k.oy = k.oz = 0;
+    } else {
+        k.base = v->dev_data + brick_id(v, bx, by, bz) * v->brick_elems;
+        k.sy = v->E; k.sz = (long long)v->E * v->E;
+        k.ox = (int)(bx * v->B); k.oy = (int)(by * v->B); k.oz = (int)(bz * v->B);
+    }
+}
+
+// ------------------------------------------------------------------ out-of-core streamer (A5)
+// Returns the device pointer of brick `b` for work enqueued on `st` right after this call and
+// makes `st` wait for its upload.  Bricks [0, n_fixed) live permanently in slot b; the others
+// pass through a ring of n_ring slots fed round-robin by the copy streams, so uploads of the
+// next bricks overlap the kernels of the current one (last sentence).
+static vr_status stream_brick_acquire(vr_volume *v, uint64_t b, cudaStream_t st, const float **ptr, uint32_t *slot_out)
+{
+    uint32_t slot;
+    bool upload;
+    if (b < v->n_fixed) { slot = (uint32_t)b; upload = !v->fixed_loaded[b]; v->fixed_loaded[b] = 1; }
+    else { slot = v->n_fixed + (uint32_t)(v->ring_pos++ % v->n_ring); upload = true; }
+    float *dst = v->pool + (size_t)slot * v->brick_elems;
+    if (upload) {
+        cudaStream_t cs = v->copy[v->copy_rr++ % (uint64_t)v->n_copy];
+        if (v->slot_used[slot]) VR_CUDA(cudaStreamWaitEvent(cs, v->ev_free[slot], 0));
+        const size_t bytes = v->brick_elems * sizeof(float);
+        VR_CUDA(cudaMemcpyAsync(dst, v->desc.data + b * v->brick_elems, bytes, cudaMemcpyHostToDevice, cs));
+        VR_CUDA(cudaEventRecord(v->ev_up[slot], cs));
+        v->stats.h2d_bytes += bytes;
+        v->slot_used[slot] = 1;
+    }
+    if (v->slot_used[slot]) VR_CUDA(cudaStreamWaitEvent(st, v->ev_up[slot], 0));
+    *ptr = dst; *slot_out = slot;
+    return VR_OK;
+}
+
+static vr_status stream_brick_release(vr_volume *v, uint32_t slot, cudaStream_t st)
+{
+    if (slot >= v->n_fixed) VR_CUDA(cudaEventRecord(v->ev_free[slot], st));
+    return VR_OK;
+}
+
+// ------------------------------------------------------------------ per-frame brick planning (A4)
+struct PlannedBrick { BrickK k; double key; uint32_t b[3]; uint64_t id; };
+
+static bool zero3(const float *a) { return a[0] == 0.0f && a[1] == 0.0f && a[2] == 0.0f; }
+
+static double det3(const double a[3], const double b[3], const double c[3])
+{
+    return a[0] * (b[1] * c[2] - b[2] * c[1]) - b[0] * (a[1] * c[2] - a[2] * c[1]) + c[0] * (a[1] * b[2] - a[2] * b[1]);
+}
+
+// conservative screen rectangle of an axis-aligned box of sample positions
+static void box_rect(const vr_camera *c, bool perspective, const double lo[3], const double hi[3], int &x0, int &y0,
+                     int &x1, int &y1)
+{
+    const int W = (int)c->width, H = (int)c->height;
+    double mnx = 1e300, mny = 1e300, mxx = -1e300, mxy = -1e300;
+    bool full = false;
+    for (int corner = 0; corner < 8 && !full; ++corner) {
+        double P[3];
+        for (int a = 0; a < 3; ++a) P[a] = (corner >> a & 1) ? hi[a] : lo[a];
+        double x, y;
+        if (perspective) {            // d0 + x du + y dv = lambda (P - o0)
+            double m0[3], m1[3], m2[3], rhs[3];
+            for (int a = 0; a < 3; ++a) { m0[a] = c->du[a]; m1[a] = c->dv[a]; m2[a] = -(P[a] - (double)c->o0[a]); rhs[a] = -(double)c->d0[a]; }
+            const double D = det3(m0, m1, m2);
+            if (std::fabs(D) < 1e-300) { full = true; break; }
+            x = det3(rhs, m1, m2) / D; y = det3(m0, rhs, m2) / D;
+            const double lambda = det3(m0, m1, rhs) / D;
+            if (!(lambda > 1e-9)) { full = true; break; }       // corner at or behind the eye
+        } else {                      // o0 + x ou + y ov + t d0 = P
+            double m0[3], m1[3], m2[3], rhs[3];
+            for (int a = 0; a < 3; ++a) { m0[a] = c->ou[a]; m1[a] = c->ov[a]; m2[a] = c->d0[a]; rhs[a] = P[a] - (double)c->o0[a]; }
+            const double D = det3(m0, m1, m2);
+            if (std::fabs(D) < 1e-300) { full = true; break; }
+            x = det3(rhs, m1, m2) / D; y = det3(m0, rhs, m2) / D;
+        }
+        if (!std::isfinite(x) || !std::isfinite(y)) { full = true; break; }
+        mnx = std::min(mnx, x); mxx = std::max(mxx, x); mny = std::min(mny, y); mxy = std::max(mxy, y);
+    }
+    if (full) { x0 = 0; y0 = 0; x1 = W; y1 = H; return; }
+    // pixel i has x = i + 0.5; one extra pixel of slack for float32 ray arithmetic
+    const double fx0 = std::floor(mnx - 0.5) - 1.0, fy0 = std::floor(mny - 0.5) - 1.0;
+    const double fx1 = std::ceil(mxx - 0.5) + 2.0, fy1 = std::ceil(mxy - 0.5) + 2.0;
+    x0 = (int)std::min(std::max(fx0, 0.0), (double)W); x1 = (int)std::min(std::max(fx1, 0.0), (double)W);
+    y0 = (int)std::min(std::max(fy0, 0.0), (double)H); y1 = (int)std::min(std::max(fy1, 0.0), (double)H);
+}
+
+// bricks that own samples and touch the screen, in visibility order (C.7)
+static void plan_bricks(const vr_volume *v, const vr_camera *c, std::vector<PlannedBrick> &out, uint32_t &culled)
+{
+    const bool perspective = zero3(c->ou) && zero3(c->ov);
+    const int n[3] = { (int)v->desc.nx, (int)v->desc.ny, (int)v->desc.nz };
+    out.clear();
+    culled = 0;
+    for (uint32_t bz = 0; bz < v->nb[2]; ++bz)
+        for (uint32_t by = 0; by < v->nb[1]; ++by)
+            for (uint32_t bx = 0; bx < v->nb[0]; ++bx) {
+                PlannedBrick p;
+                p.b[0] = bx; p.b[1] = by; p.b[2] = bz; p.id = brick_id(v, bx, by, bz);
+                bool empty = false;
+                double lo[3], hi[3];
+                p.key = 0.0;
+                for (int a = 0; a < 3; ++a) {
+                    owned_range(v, a, p.b[a], p.k.lo[a], p.k.hi[a]);
+                    if (p.k.lo[a] > p.k.hi[a]) empty = true;
+                    // ownership cell in position space, outer cells reach the volume faces; 0.01 voxel slack
+                    lo[a] = (p.k.lo[a] == 0 ? 0.0 : p.k.lo[a] + 0.5) - 0.01;
+                    hi[a] = (p.k.hi[a] == n[a] - 2 ? (double)n[a] : p.k.hi[a] + 1.5) + 0.01;
+                    const double centre = (double)v->B * (p.b[a] + 0.5) + 0.5;      // ownership-lattice centre
+                    if (perspective) { const double e = (double)c->o0[a] - centre; p.key += e * e; }
+                    else p.key += centre * (double)c->d0[a];
+                }
+                if (empty) continue;
+                box_rect(c, perspective, lo, hi, p.k.x0, p.k.y0, p.k.x1, p.k.y1);
+                if (p.k.x1 <= p.k.x0 || p.k.y1 <= p.k.y0) { ++culled; continue; }
+                p.k.frag_off = 0;
+                p.k.base = nullptr; p.k.sy = p.k.sz = 0; p.k.ox = p.k.oy = p.k.oz = 0;
+                out.push_back(p);
+            }
+    std::stable_sort(out.begin(), out.end(), [](const PlannedBrick &a, const PlannedBrick &b) { return a.key < b.key; });
+}
+
+static vr_status staging_acquire(vr_volume *v, size_t bytes, Staging **out)
+{
+    Staging &s = v->staging[v->staging_next];
+    v->staging_next = (v->staging_next + 1) % kStagingRing;
+    if (!s.done) VR_CUDA(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+    if (s.in_flight) { VR_CUDA(cudaEventSynchronize(s.done)); s.in_flight = false; }
+    if (bytes > s.cap) {
+        if (s.h) { VR_CUDA(cudaFreeHost(s.h)); s.h = nullptr; }
+        if (s.d) { VR_CUDA(cudaFree(s.d)); s.d = nullptr; }
+        s.cap = 0;
+        const size_t want = bytes + bytes / 2 + 4096;
+        VR_CUDA(cudaMallocHost(&s.h, want));
+        VR_CUDA(cudaMalloc(&s.d, want));
+        s.cap = want;
+    }
+    *out = &s;
+    return VR_OK;
+}
+
+static CamK to_camk(const vr_camera *c)
+{
+    CamK k;
+    for (int a = 0; a < 3; ++a) {
+        k.o0[a] = c->o0[a]; k.ou[a] = c->ou[a]; k.ov[a] = c->ov[a];
+        k.d0[a] = c->d0[a]; k.du[a] = c->du[a]; k.dv[a] = c->dv[a];
+    }
+    k.step = c->step;
+    k.t_min = 1.0f - c->ert_alpha;        // one float32 subtraction (C.5)
+    k.width = (int)c->width; k.height = (int)c->height;
+    return k;
+}
+
+// ------------------------------------------------------------------ render paths
+static vr_status render_single(vr_volume *v, const CamK &cam, int mode, bool ert, const TfK &tf, float *img,
+                               long long pitch_f, cudaStream_t st)
+{
+    VolK V;
+    V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
+    V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz; V.ox = V.oy = V.oz = 0;
+    launch_march_full(mode, ert, cam, V, tf, img, pitch_f, st);
+    v->stats.kernel_launches += 1;
+    v->stats.path = 1;
+    v->stats.bricks_drawn = (uint32_t)v->n_bricks;
+    return VR_OK;
+}
+
+static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, const TfK &tf,
+                                  float *img, long long pitch_f, cudaStream_t st)
+{
+    std::vector<PlannedBrick> plan;
+    uint32_t culled = 0;
+    plan_bricks(v, c, plan, culled);
+    const int W = cam.width, H = cam.height;
+    const int bins_x = (W + 15) / 16, bins_y = (H + 15) / 16;
+    // fragments, work items, bins
+    uint64_t n_frag = 0;
+    size_t n_work = 0;
+    std::vector<uint32_t> bin_cnt((size_t)bins_x * bins_y + 1, 0);
+    for (auto &p : plan) {
+        resident_brick_view(v, p.b[0], p.b[1], p.b[2], p.k);
+        p.k.frag_off = n_frag;
+        const int w = p.k.x1 - p.k.x0, h = p.k.y1 - p.k.y0;
+        n_frag += (uint64_t)w * h;
+        n_work += (size_t)((w + 15) / 16) * ((h + 7) / 8);
+        for (int ty = p.k.y0 / 16; ty <= (p.k.y1 - 1) / 16; ++ty)
+            for (int tx = p.k.x0 / 16; tx <= (p.k.x1 - 1) / 16; ++tx) bin_cnt[(size_t)ty * bins_x + tx]++;
+    }
+    size_t n_list = 0;
+    for (size_t i = 0; i < bin_cnt.size(); ++i) { const uint32_t c2 = bin_cnt[i]; bin_cnt[i] = (uint32_t)n_list; n_list += c2; }
+    if (n_work > 0x7fffffffull) { set_error("too many (brick, tile) work items: %zu", n_work); return VR_ERR_UNSUPPORTED; }
+
+    const size_t off_bricks = 0;
+    const size_t off_work = (off_bricks + plan.size() * sizeof(BrickK) + 255) & ~(size_t)255;
+    const size_t off_offs = (off_work + n_work * sizeof(WorkK) + 255) & ~(size_t)255;
+    const size_t off_list = (off_offs + bin_cnt.size() * sizeof(uint32_t) + 255) & ~(size_t)255;
+    const size_t total = off_list + n_list * sizeof(uint32_t) + 256;
+    Staging *s;
+    vr_status rc = staging_acquire(v, total, &s);
+    if (rc != VR_OK) return rc;
+    BrickK *hb = reinterpret_cast<BrickK *>(s->h + off_bricks);
+    WorkK *hw = reinterpret_cast<WorkK *>(s->h + off_work);
+    uint32_t *ho = reinterpret_cast<uint32_t *>(s->h + off_offs);
+    uint32_t *hl = reinterpret_cast<uint32_t *>(s->h + off_list);
+    std::vector<uint32_t> fill(bin_cnt.begin(), bin_cnt.end() - 1);
+    size_t wi = 0;
+    for (size_t bi = 0; bi < plan.size(); ++bi) {
+        const BrickK &k = plan[bi].k;
+        hb[bi] = k;
+        const int tw = (k.x1 - k.x0 + 15) / 16, th = (k.y1 - k.y0 + 7) / 8;
+        for (int ty = 0; ty < th; ++ty)
+            for (int tx = 0; tx < tw; ++tx) { hw[wi].brick = (int)bi; hw[wi].tx = tx; hw[wi].ty = ty; hw[wi].pad = 0; ++wi; }
+        for (int ty = k.y0 / 16; ty <= (k.y1 - 1) / 16; ++ty)
+            for (int tx = k.x0 / 16; tx <= (k.x1 - 1) / 16; ++tx) hl[fill[(size_t)ty * bins_x + tx]++] = (uint32_t)bi;
+    }
+    memcpy(ho, bin_cnt.data(), bin_cnt.size() * sizeof(uint32_t));
+
+    rc = v->arena.reserve((size_t)n_frag * (mode == VR_EA ? 4 : 1) + 4);
+    if (rc != VR_OK) return rc;
+    VR_CUDA(cudaMemcpyAsync(s->d, s->h, total, cudaMemcpyHostToDevice, st));
+    v->stats.h2d_bytes += total;
+
+    VolK Vdims;                               // dims only; base / strides / origin come from each BrickK
+    Vdims.nx = (int)v->desc.nx; Vdims.ny = (int)v->desc.ny; Vdims.nz = (int)v->desc.nz;
+    Vdims.base = nullptr; Vdims.sy = Vdims.sz = 0; Vdims.ox = Vdims.oy = Vdims.oz = 0;
+    // 64-bit element offsets only when a linear volume exceeds 2^32-1 voxels; slots never do
+    const bool wide = v->desc.layout == VR_LINEAR && v->n_vox > 0xffffffffull;
+    launch_march_bricks(mode, wide, cam, Vdims, tf, reinterpret_cast<const BrickK *>(s->d + off_bricks),
+                        reinterpret_cast<const WorkK *>(s->d + off_work), (int)n_work, v->arena.p, st);
+    BinsK bins;
+    bins.offs = reinterpret_cast<const unsigned int *>(s->d + off_offs);
+    bins.list = reinterpret_cast<const unsigned int *>(s->d + off_list);
+    bins.tiles_x = bins_x; bins.tile = 16;
+    launch_composite(mode, cam, reinterpret_cast<const BrickK *>(s->d + off_bricks), bins, v->arena.p, img, pitch_f, st);
+    VR_CUDA(cudaEventRecord(s->done, st));
+    s->in_flight = true;
+    v->stats.kernel_launches += (n_work ? 1 : 0) + 1;
+    v->stats.path = 2;
+    v->stats.fragments = n_frag;
+    v->stats.bricks_drawn = (uint32_t)plan.size();
+    v->stats.bricks_culled = culled;
+    return VR_OK;
+}
+
+// brick-by-brick front to back, ray state carried in the image (exact ERT).  Used for every
+// out-of-core volume and for resident VR_BRICKED_HALO1 volumes without VR_SORT_LAST.
+static vr_status render_chain(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, const TfK &tf,
+                              float *img, long long pitch_f, cudaStream_t st)
+{
+    std::vector<PlannedBrick> plan;
+    uint32_t culled = 0;
+    plan_bricks(v, c, plan, culled);
+    VolK V;
+    V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz;
+    V.base = nullptr; V.sy = V.sz = 0; V.ox = V.oy = V.oz = 0;
+    launch_chain_init(mode, cam.width, cam.height, img, pitch_f, st);
+    v->stats.kernel_launches += 1;
+    for (auto &p : plan) {
+        uint32_t slot = 0;
+        if (v->out_of_core) {
+            const float *ptr;
+            vr_status rc = stream_brick_acquire(v, p.id, st, &ptr, &slot);
+            if (rc != VR_OK) return rc;
+            p.k.base = ptr; p.k.sy = v->E; p.k.sz = (long long)v->E * v->E;
+            p.k.ox = (int)(p.b[0] * v->B); p.k.oy = (int)(p.b[1] * v->B); p.k.oz = (int)(p.b[2] * v->B);
+        } else resident_brick_view(v, p.b[0], p.b[1], p.b[2], p.k);
+        launch_chain_brick(mode, ert, cam, V, tf, p.k, img, pitch_f, st);
+        v->stats.kernel_launches += 1;
+        if (v->out_of_core) { vr_status rc = stream_brick_release(v, slot, st); if (rc != VR_OK) return rc; }
+    }
+    if (mode == VR_EA) { launch_chain_finish(cam.width, cam.height, img, pitch_f, st); v->stats.kernel_launches += 1; }
+    v->stats.path = 3;
+    v->stats.bricks_drawn = (uint32_t)plan.size();
+    v->stats.bricks_culled = culled;
+    return VR_OK;
+}
+
+}  // namespace vr
+
+// ====================================================================== C ABI
+extern "C" {
+
+VR_API const char *vr_last_error(void) { return g_err; }
+VR_API const char *vr_version(void) { return "vr-b200 0.1 sm_100a"; }
+
+VR_API vr_status vr_create_volume(const vr_volume_desc *d, vr_volume **out)
+{
+    g_err[0] = 0;
+    VR_REQUIRE(d && out, "vr_create_volume: NULL argument");
+    *out = nullptr;
+    VR_REQUIRE(d->struct_size == sizeof(vr_volume_desc), "vr_volume_desc.struct_size %u != %zu", d->struct_size, sizeof(vr_volume_desc));
+    VR_REQUIRE(d->nx >= 2 && d->ny >= 2 && d->nz >= 2, "each dimension must be >= 2 (got %ux%ux%u)", d->nx, d->ny, d->nz);
+    VR_REQUIRE(d->nx <= 0x7fffffffu && d->ny <= 0x7fffffffu && d->nz <= 0x7fffffffu, "dimension too large");
+    VR_REQUIRE(d->layout == VR_LINEAR || d->layout == VR_BRICKED_HALO1, "bad layout %u", d->layout);
+    VR_REQUIRE(d->location == VR_DEVICE || d->location == VR_HOST_PINNED, "bad location %u", d->location);
+    VR_REQUIRE(d->data != nullptr, "data is NULL");
+    VR_REQUIRE(d->layout == VR_LINEAR || d->brick > 0, "VR_BRICKED_HALO1 needs brick > 0");
+    VR_REQUIRE(d->n_copy_streams <= (uint32_t)kMaxCopyStreams, "n_copy_streams must be <= %d", kMaxCopyStreams);
+    VR_REQUIRE(((uintptr_t)d->data & 15u) == 0, "data must be 16-byte aligned");
+
+    vr_volume *v = new (std::nothrow) vr_volume();
+    if (!v) { set_error("host allocation failed"); return VR_ERR_OUT_OF_MEMORY; }
+    v->desc = *d;
+    memset(&v->stats, 0, sizeof(v->stats));
+    v->stats.struct_size = sizeof(vr_stats);
+    const uint32_t maxdim = std::max(d->nx, std::max(d->ny, d->nz));
+    v->B = d->brick ? d->brick : maxdim;
+    v->E = v->B + 1;
+    const uint32_t n[3] = { d->nx, d->ny, d->nz };
+    for (int a = 0; a < 3; ++a) v->nb[a] = d->brick ? (n[a] + v->B - 1) / v->B : 1;
+    if (v->nb[0] > 65535 || v->nb[1] > 65535 || v->nb[2] > 65535) {
+        delete v; set_error("brick grid exceeds 65535 bricks on an axis"); return VR_ERR_INVALID_ARG;
+    }
+    v->n_bricks = (uint64_t)v->nb[0] * v->nb[1] * v->nb[2];
+    v->n_vox = (uint64_t)d->nx * d->ny * d->nz;
+    v->brick_elems = (uint64_t)v->E * v->E * v->E;
+    v->total_elems = d->layout == VR_LINEAR ? v->n_vox : v->n_bricks * v->brick_elems;
+    v->stats.n_bricks = (uint32_t)std::min<uint64_t>(v->n_bricks, 0xffffffffu);
+
+#define VR_FAIL_CUDA(call)                                                   \
+    do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { vr_status r__ = cuda_fail(e__, #call); free_volume(v); return r__; } } while (0)
+
+    VR_FAIL_CUDA(cudaGetDevice(&v->device));
+    VR_FAIL_CUDA(cudaDeviceGetAttribute(&v->sm_count, cudaDevAttrMultiProcessorCount, v->device));
+    cudaPointerAttributes attr;
+    VR_FAIL_CUDA(cudaPointerGetAttributes(&attr, d->data));
+    if (d->location == VR_DEVICE) {
+        if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged) {
+            free_volume(v); set_error("location VR_DEVICE but data is not a device pointer"); return VR_ERR_INVALID_ARG;
+        }
+        v->dev_data = d->data;
+    } else {
+        if (attr.type != cudaMemoryTypeHost) {
+            free_volume(v); set_error("location VR_HOST_PINNED but data is not page-locked host memory"); return VR_ERR_INVALID_ARG;
+        }
+        v->n_copy = d->n_copy_streams ? (int)d->n_copy_streams : 4;
+        for (int i = 0; i < v->n_copy; ++i) VR_FAIL_CUDA(cudaStreamCreateWithFlags(&v->copy[i], cudaStreamNonBlocking));
+        const uint64_t bytes = v->total_elems * sizeof(float);
+        if (d->resident_bytes == 0 || d->resident_bytes >= bytes) {
+            VR_FAIL_CUDA(cudaMalloc(&v->mirror, bytes));
+            v->dev_data = v->mirror;
+            v->mirror_ev.resize(v->n_copy);
+            for (auto &e : v->mirror_ev) VR_FAIL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            v->stats.resident_bytes = bytes;
+        } else {
+            if (d->layout != VR_BRICKED_HALO1) {
+                free_volume(v); set_error("out-of-core streaming (resident_bytes < volume bytes) needs VR_BRICKED_HALO1");
+                return VR_ERR_UNSUPPORTED;
+            }
+            const uint64_t bb = v->brick_elems * sizeof(float);
+            v->n_slots = (uint32_t)std::min<uint64_t>(d->resident_bytes / bb, v->n_bricks);
+            if (v->n_slots < 2) { free_volume(v); set_error("resident_bytes holds fewer than 2 bricks of %llu bytes", (unsigned long long)bb); return VR_ERR_INVALID_ARG; }
+            v->n_ring = std::min<uint32_t>(v->n_slots, std::max<uint32_t>(2u, 2u * (uint32_t)v->n_copy));
+            v->n_fixed = v->n_slots - v->n_ring;
+            v->out_of_core = true;
+            VR_FAIL_CUDA(cudaMalloc(&v->pool, (size_t)v->n_slots * bb));
+            v->fixed_loaded.assign(v->n_fixed, 0);
+            v->slot_used.assign(v->n_slots, 0);
+            v->ev_up.resize(v->n_slots); v->ev_free.resize(v->n_slots);
+            for (auto &e : v->ev_up) VR_FAIL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            for (auto &e : v->ev_free) VR_FAIL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            v->stats.resident_bytes = (uint64_t)v->n_slots * bb;
+        }
+    }
+    VR_FAIL_CUDA(cudaMalloc(&v->d_tf, 257 * sizeof(float4)));
+    VR_FAIL_CUDA(cudaMalloc(&v->d_sum, sizeof(SummaryScratch)));
+    VR_FAIL_CUDA(cudaMalloc(&v->d_sum_out, VR_SUMMARY_BYTES(4096)));
+#undef VR_FAIL_CUDA
+    *out = v;
+    return VR_OK;
+}
+
+VR_API vr_status vr_destroy_volume(vr_volume *v)
+{
+    g_err[0] = 0;
+    free_volume(v);
+    return VR_OK;
+}
+
+VR_API vr_status vr_set_transfer_function(vr_volume *v, const float *rgba, float vmin, float vmax)
+{
+    g_err[0] = 0;
+    VR_REQUIRE(v && rgba, "vr_set_transfer_function: NULL argument");
+    VR_REQUIRE(std::isfinite(vmin) && std::isfinite(vmax) && vmax > vmin, "need finite vmin < vmax (got %g, %g)", vmin, vmax);
+    float tab[257 * 4];
+    for (int i = 0; i < 1024; ++i) {
+        VR_REQUIRE(std::isfinite(rgba[i]) && rgba[i] >= 0.0f && rgba[i] <= 1.0f, "table entry %d = %g is outside [0,1]", i, rgba[i]);
+        tab[i] = rgba[i];
+    }
+    for (int c = 0; c < 4; ++c) tab[1024 + c] = rgba[1020 + c];      // pad entry (never weighted: i <= 254)
+    VR_CUDA(cudaSetDevice(v->device));
+    VR_CUDA(cudaMemcpy(v->d_tf, tab, sizeof(tab), cudaMemcpyHostToDevice));
+    v->tf_scale = 1.0f / (vmax - vmin);                             // C.4, float32
+    v->tf_bias = -vmin * v->tf_scale;
+    v->tf_set = true;
+    return VR_OK;
+}
+
+VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_image *im, void *stream)
+{
+    g_err[0] = 0;
+    VR_REQUIRE(v && c && im, "vr_render: NULL argument");
+    VR_REQUIRE(c->struct_size == sizeof(vr_camera), "vr_camera.struct_size %u != %zu", c->struct_size, sizeof(vr_camera));
+    VR_REQUIRE(im->struct_size == sizeof(vr_image), "vr_image.struct_size %u != %zu", im->struct_size, sizeof(vr_image));
+    VR_REQUIRE(mode == VR_EA || mode == VR_MIP, "bad mode %d", mode);
+    VR_REQUIRE(c->width > 0 && c->height > 0 && c->width <= 65536 && c->height <= 65536, "bad image size %ux%u", c->width, c->height);
+    VR_REQUIRE(std::isfinite(c->step) && c->step > 0.0f, "step must be finite and > 0 (got %g)", c->step);
+    VR_REQUIRE(c->ert_alpha >= 0.0f && c->ert_alpha < 1.0f, "ert_alpha must be in [0,1) (got %g)", c->ert_alpha);
+    for (int a = 0; a < 3; ++a)
+        VR_REQUIRE(std::isfinite(c->o0[a]) && std::isfinite(c->ou[a]) && std::isfinite(c->ov[a]) && std::isfinite(c->d0[a]) &&
+                   std::isfinite(c->du[a]) && std::isfinite(c->dv[a]), "camera vectors must be finite");
+    const uint32_t ch = mode == VR_EA ? 4u : 1u;
+    VR_REQUIRE(im->channels == ch, "image.channels %u does not match mode (%u expected)", im->channels, ch);
+    VR_REQUIRE(im->pixels != nullptr, "image.pixels is NULL");
+    VR_REQUIRE(im->location == VR_DEVICE || im->location == VR_HOST_PINNED, "bad image.location %u", im->location);
+    const uint64_t row_bytes = (uint64_t)c->width * ch * 4;
+    const uint64_t pitch = im->row_pitch_bytes ? im->row_pitch_bytes : row_bytes;
+    VR_REQUIRE(pitch >= row_bytes && pitch % (mode == VR_EA ? 16 : 4) == 0, "bad row_pitch_bytes %llu", (unsigned long long)pitch);
+    VR_REQUIRE(((uintptr_t)im->pixels & (mode == VR_EA ? 15u : 3u)) == 0, "image.pixels is misaligned");
+    if (mode == VR_EA && !v->tf_set) { set_error("emission-absorption render before vr_set_transfer_function"); return VR_ERR_NOT_READY; }
+    const bool sort_last = (c->flags & VR_SORT_LAST) != 0;
+    const bool ert = mode == VR_EA && c->ert_alpha > 0.0f;
+    const bool persp = zero3(c->ou) && zero3(c->ov), ortho = zero3(c->du) && zero3(c->dv);
+    if (sort_last) {
+        if (!v->desc.brick) { set_error("VR_SORT_LAST needs a bricked volume (brick > 0)"); return VR_ERR_UNSUPPORTED; }
+        if (ert) { set_error("early ray termination is not defined for independent per-brick partials (S15)"); return VR_ERR_UNSUPPORTED; }
+        if (v->out_of_core) { set_error("VR_SORT_LAST is not available for out-of-core volumes (they render as a chain)"); return VR_ERR_UNSUPPORTED; }
+    }
+    const bool need_plan = sort_last || v->out_of_core || v->desc.layout == VR_BRICKED_HALO1;
+    if (need_plan && !persp && !ortho) { set_error("bricked rendering needs a pure perspective or pure orthographic camera"); return VR_ERR_UNSUPPORTED; }
+
+    VR_CUDA(cudaSetDevice(v->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    v->stats.kernel_launches = 0; v->stats.h2d_bytes = 0; v->stats.d2h_bytes = 0; v->stats.fragments = 0;
+    v->stats.bricks_drawn = v->stats.bricks_culled = 0;
+
+    float *img = im->pixels;
+    long long pitch_f = (long long)(pitch / 4);
+    if (im->location == VR_HOST_PINNED) {
+        vr_status rc = v->host_image.reserve((size_t)c->width * c->height * ch);
+        if (rc != VR_OK) return rc;
+        img = v->host_image.p; pitch_f = (long long)c->width * ch;
+    }
+    vr_status rc = ensure_mirror(v, st);
+    if (rc != VR_OK) return rc;
+
+    const CamK cam = to_camk(c);
+    TfK tf; tf.table = v->d_tf; tf.scale = v->tf_scale; tf.bias = v->tf_bias;
+    if (sort_last) rc = render_sort_last(v, c, cam, mode, tf, img, pitch_f, st);
+    else if (v->out_of_core || v->desc.layout == VR_BRICKED_HALO1) rc = render_chain(v, c, cam, mode, ert, tf, img, pitch_f, st);
+    else rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
+    if (rc != VR_OK) return rc;
+    VR_CUDA(cudaGetLastError());
+    if (im->location == VR_HOST_PINNED) {
+        if (pitch == row_bytes) VR_CUDA(cudaMemcpyAsync(im->pixels, img, row_bytes * c->height, cudaMemcpyDeviceToHost, st));
+        else VR_CUDA(cudaMemcpy2DAsync(im->pixels, pitch, img, row_bytes, row_bytes, c->height, cudaMemcpyDeviceToHost, st));
+        v->stats.d2h_bytes += row_bytes * c->height;
+    }
+    v->stats.total_kernel_launches += v->stats.kernel_launches;
+    return VR_OK;
+}
+
+VR_API vr_status vr_minmax_histogram(vr_volume *v, uint32_t nbins, const float *range, vr_summary *out,
+                                     uint32_t out_location, void *stream)
+{
+    g_err[0] = 0;
+    VR_REQUIRE(v && out, "vr_minmax_histogram: NULL argument");
+    VR_REQUIRE(nbins >= 1 && nbins <= 4096, "nbins must be in 1..4096 (got %u)", nbins);
+    VR_REQUIRE(out_location == VR_DEVICE || out_location == VR_HOST_PINNED, "bad out_location %u", out_location);
+    VR_REQUIRE(((uintptr_t)out & 7u) == 0, "out must be 8-byte aligned");
+    float lo = 0.0f, hi = 0.0f;
+    if (range) {
+        lo = range[0]; hi = range[1];
+        VR_REQUIRE(std::isfinite(lo) && std::isfinite(hi) && hi >= lo, "range must be finite with range[1] >= range[0]");
+    }
+    VR_CUDA(cudaSetDevice(v->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    v->stats.kernel_launches = 0; v->stats.h2d_bytes = 0; v->stats.d2h_bytes = 0;
+    vr_status rc = ensure_mirror(v, st);
+    if (rc != VR_OK) return rc;
+    const int grid = v->sm_count * 2;
+    SummaryScratch *S = v->d_sum;
+    launch_summary_reset(S, st);
+    v->stats.kernel_launches += 1;
+    const int n_pass = range ? 1 : 2;
+    const uint32_t n[3] = { v->desc.nx, v->desc.ny, v->desc.nz };
+    for (int pass = 0; pass < n_pass; ++pass) {
+        // pass 0: min/max (+ histogram when the caller gave the range); pass 1: histogram over [min,max]
+        if (range && pass == 0) { launch_summary_range(S, 1, lo, hi, nbins, st); v->stats.kernel_launches += 1; }
+        if (pass == 1) { launch_summary_range(S, 0, 0.0f, 0.0f, nbins, st); v->stats.kernel_launches += 1; }
+        if (v->desc.layout == VR_LINEAR) {
+            if (pass == 1) launch_hist_flat(v->dev_data, v->n_vox, nbins, S, grid, st);
+            else if (range) launch_minmax_hist_flat(v->dev_data, v->n_vox, nbins, S, grid, st);
+            else launch_minmax_flat(v->dev_data, v->n_vox, S, grid, st);
+            v->stats.kernel_launches += 1;
+        } else {
+            for (uint32_t bz = 0; bz < v->nb[2]; ++bz)
+                for (uint32_t by = 0; by < v->nb[1]; ++by)
+                    for (uint32_t bx = 0; bx < v->nb[0]; ++bx) {
+                        const uint64_t id = brick_id(v, bx, by, bz);
+                        BoxK box;
+                        uint32_t slot = 0;
+                        if (v->out_of_core) {
+                            const float *ptr;
+                            rc = stream_brick_acquire(v, id, st, &ptr, &slot);
+                            if (rc != VR_OK) return rc;
+                            box.base = ptr;
+                        } else box.base = v->dev_data + id * v->brick_elems;
+                        box.sy = v->E; box.sz = (long long)v->E * v->E;
+                        const uint32_t bb[3] = { bx, by, bz };
+                        int ext[3];
+                        for (int a = 0; a < 3; ++a) ext[a] = (int)std::min(v->B, n[a] - bb[a] * v->B);   // halo excluded
+                        box.ex = ext[0]; box.ey = ext[1]; box.ez = ext[2];
+                        const int bgrid = (int)std::min<long long>(grid, ((long long)box.ey * box.ez + 15) / 16);
+                        if (pass == 1) launch_hist_box(box, nbins, S, bgrid, st);
+                        else if (range) launch_minmax_hist_box(box, nbins, S, bgrid, st);
+                        else launch_minmax_box(box, S, bgrid, st);
+                        v->stats.kernel_launches += 1;
+                        if (v->out_of_core) { rc = stream_brick_release(v, slot, st); if (rc != VR_OK) return rc; }
+                    }
+        }
+    }
+    if (out_location == VR_DEVICE) launch_summary_finish(S, nbins, out, st);
+    else {
+        launch_summary_finish(S, nbins, v->d_sum_out, st);
+        VR_CUDA(cudaMemcpyAsync(out, v->d_sum_out, VR_SUMMARY_BYTES(nbins), cudaMemcpyDeviceToHost, st));
+        v->stats.d2h_bytes += VR_SUMMARY_BYTES(nbins);
+    }
+    v->stats.kernel_launches += 1;
+    VR_CUDA(cudaGetLastError());
+    v->stats.total_kernel_launches += v->stats.kernel_launches;
+    return VR_OK;
+}
+
+VR_API vr_status vr_get_stats(vr_volume *v, vr_stats *s)
+{
+    g_err[0] = 0;
+    VR_REQUIRE(v && s, "vr_get_stats: NULL argument");
+    VR_REQUIRE(s->struct_size == sizeof(vr_stats), "vr_stats.struct_size %u != %zu", s->struct_size, sizeof(vr_stats));
+    *s = v->stats;
+    return VR_OK;
+}
+
+}  // extern "C"

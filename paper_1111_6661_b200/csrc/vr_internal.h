@@ -1,0 +1,84 @@
+// vr_internal.h — host-side handle, error plumbing and kernel launcher declarations.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/vr.h"
+#include "vr_math.cuh"
+
+namespace vr {
+
+void set_error(const char *fmt, ...);
+vr_status cuda_fail(cudaError_t e, const char *what);
+
+#define VR_CUDA(call)                                                  \
+    do {                                                               \
+        cudaError_t e__ = (call);                                      \
+        if (e__ != cudaSuccess) return ::vr::cuda_fail(e__, #call);    \
+    } while (0)
+
+#define VR_REQUIRE(cond, ...)                                          \
+    do {                                                               \
+        if (!(cond)) { ::vr::set_error(__VA_ARGS__); return VR_ERR_INVALID_ARG; } \
+    } while (0)
+
+// ---------------------------------------------------------------- reductions (vr_reduce.cu)
+// device scratch of one summary call
+struct SummaryScratch {
+    unsigned int enc_min, enc_max;        // order-preserving uint encodings of the running min / max
+    float lo, hi, scale_h;                // histogram range decided on the device
+    unsigned int pad;
+    unsigned long long n_nonfinite, n_below, n_above;
+    unsigned long long counts[4096];
+};
+
+struct BoxK {                             // a box of voxels inside a strided array
+    const float *base;
+    long long sy, sz;
+    int ex, ey, ez;
+};
+
+void launch_summary_reset(SummaryScratch *s, cudaStream_t st);
+void launch_minmax_flat(const float *v, unsigned long long n, SummaryScratch *s, int grid, cudaStream_t st);
+void launch_minmax_box(BoxK b, SummaryScratch *s, int grid, cudaStream_t st);
+// range_mode 0: lo/hi = the device min/max; 1: lo/hi given
+void launch_summary_range(SummaryScratch *s, int range_mode, float lo, float hi, uint32_t nbins, cudaStream_t st);
+void launch_hist_flat(const float *v, unsigned long long n, uint32_t nbins, SummaryScratch *s, int grid, cudaStream_t st);
+void launch_hist_box(BoxK b, uint32_t nbins, SummaryScratch *s, int grid, cudaStream_t st);
+// fused single pass (caller gave the range): min/max and histogram together
+void launch_minmax_hist_flat(const float *v, unsigned long long n, uint32_t nbins, SummaryScratch *s, int grid,
+                             cudaStream_t st);
+void launch_minmax_hist_box(BoxK b, uint32_t nbins, SummaryScratch *s, int grid, cudaStream_t st);
+void launch_summary_finish(const SummaryScratch *s, uint32_t nbins, vr_summary *out, cudaStream_t st);
+
+// ---------------------------------------------------------------- ray casting (vr_raycast.cu)
+struct TfK { const float4 *table; float scale, bias; };   // 257 float4 entries in global memory
+
+// one brick as the kernels see it (per-frame table, visibility order)
+struct BrickK {
+    const float *base;          // voxel (ox,oy,oz)
+    long long sy, sz;
+    int ox, oy, oz;             // index origin of base
+    int lo[3], hi[3];           // owned base-index range, inclusive (C.7): i0_a in [lo_a, hi_a]
+    int x0, y0, x1, y1;         // screen rectangle, [x0,x1) x [y0,y1)
+    unsigned long long frag_off;   // first fragment of this brick in the arena (sort-last)
+};
+
+struct WorkK { int brick, tx, ty, pad; };   // one CTA of the brick kernel: 16x8 pixel tile at (tx,ty)
+
+struct BinsK { const unsigned int *offs; const unsigned int *list; int tiles_x, tile; };
+
+void launch_march_full(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, float *image,
+                       long long pitch_f, cudaStream_t st);
+void launch_march_bricks(int mode, bool wide, const CamK &cam, const VolK &vol, const TfK &tf, const BrickK *bricks,
+                         const WorkK *work, int n_work, float *arena, cudaStream_t st);
+void launch_composite(int mode, const CamK &cam, const BrickK *bricks, BinsK bins, const float *arena, float *image,
+                      long long pitch_f, cudaStream_t st);
+void launch_chain_init(int mode, int W, int H, float *image, long long pitch_f, cudaStream_t st);
+void launch_chain_brick(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, const BrickK &brick,
+                        float *image, long long pitch_f, cudaStream_t st);
+void launch_chain_finish(int W, int H, float *image, long long pitch_f, cudaStream_t st);
+
+}  // namespace vr

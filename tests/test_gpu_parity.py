@@ -1,0 +1,249 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Bit-exact for min/max and counts, MIP <= 1e-6 scale-relative,
+EA <= 1e-4 absolute per channel (north_star)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+import paper_1111_6661_b200 as vr
+import workload as W
+from parity import check_ea, check_mip
+
+pytestmark = pytest.mark.gpu
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def pinned(a):
+    t = torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    return t
+
+
+def gpu_summary(vol, nbins=256, range_=None):
+    buf = vol.minmax_histogram(nbins, range_)
+    return vr.Volume.read_summary(buf, nbins)
+
+
+def assert_summary_equal(g, o):
+    assert g["vmin"] == o.vmin and g["vmax"] == o.vmax, (g["vmin"], o.vmin, g["vmax"], o.vmax)
+    assert int(g["n_nonfinite"]) == o.n_nonfinite and int(g["n_below"]) == o.n_below and int(g["n_above"]) == o.n_above
+    assert np.array_equal(g["counts"], o.counts)
+
+
+# ------------------------------------------------------------------ A1 / A2
+@pytest.mark.parametrize("dims", [(128, 128, 128), (37, 29, 41), (130, 67, 3), (2, 2, 2)])
+def test_minmax_hist_bit_exact(dims):
+    nx, ny, nz = dims
+    v = W.make_cube(W.Recipe(nx, ny, nz, seed=21, n_sources=4 if nx > 8 else 0))
+    # the flat kernel needs a 16-byte aligned base: torch allocations are
+    with vr.Volume(dev(v), dims) as vol:
+        assert_summary_equal(gpu_summary(vol), O.minmax_hist(v))
+        assert_summary_equal(gpu_summary(vol, 64, (-1.0, 1.5)), O.minmax_hist(v, 64, (-1.0, 1.5)))
+        assert_summary_equal(gpu_summary(vol, 1000), O.minmax_hist(v, 1000))
+        assert_summary_equal(gpu_summary(vol, 4096, (0.0, 0.0)), O.minmax_hist(v, 4096, (0.0, 0.0)))
+
+
+def test_minmax_hist_nonfinite_and_constant():
+    v = W.make_cube(W.Recipe(40, 33, 27, seed=5)).copy()
+    v[0, 0, 0], v[5, 6, 7], v[26, 32, 39], v[13, 1, 2] = np.nan, np.inf, -np.inf, np.nan
+    with vr.Volume(dev(v), (40, 33, 27)) as vol:
+        g, o = gpu_summary(vol), O.minmax_hist(v)
+        assert_summary_equal(g, o)
+        assert int(g["counts"].sum() + g["n_below"] + g["n_above"] + g["n_nonfinite"]) == v.size
+    c = np.full((9, 10, 11), 3.5, dtype=np.float32)
+    with vr.Volume(dev(c), (11, 10, 9)) as vol:
+        assert_summary_equal(gpu_summary(vol), O.minmax_hist(c))
+    k = (np.arange(8 * 16 * 32) % 256).astype(np.float32).reshape(8, 16, 32)
+    with vr.Volume(dev(k), (32, 16, 8)) as vol:
+        g = gpu_summary(vol)
+        assert np.all(g["counts"] == k.size // 256)
+
+
+# ------------------------------------------------------------------ cfg1 (full size): A3, A6-A9
+def test_cfg1_full():
+    cfg = W.get_config(1)
+    v = W.make_cube(cfg.recipe)
+    cam = cfg.camera()
+    o_sum = O.minmax_hist(v)
+    tf = W.tf_haze(cfg.dims, cfg.step)
+    with vr.Volume(dev(v), cfg.dims) as vol:
+        g = gpu_summary(vol)
+        assert_summary_equal(g, o_sum)
+        vol.set_transfer_function(tf, float(g["vmin"]), float(g["vmax"]))
+        mip = vol.render(cam, vr.VR_MIP).cpu().numpy()
+        ea = vol.render(cam, vr.VR_EA).cpu().numpy()
+        ea2 = vol.render(cam, vr.VR_EA).cpu().numpy()
+        st = vol.stats()
+    R = float(max(abs(o_sum.vmin), abs(o_sum.vmax)))
+    om = O.render(v, cam, O.MIP)
+    oe = O.render(v, cam, O.EA, tf, o_sum.vmin, o_sum.vmax)
+    sm = check_mip(mip, om.image, R)
+    se = check_ea(ea, oe.image)
+    assert sm["bit_exact"] == 1.0 and se["bit_exact"] == 1.0        # same canonical op sequence
+    assert np.array_equal(ea, ea2)                                   # run-to-run determinism
+    assert st["path"] == 1 and st["kernel_launches"] == 1
+
+
+def _views(n):
+    c = np.array(n) / 2
+    yield "persp", W.perspective_camera(c + np.array([1.9, 0.8, 1.5]) * max(n), c, (0, 1, 0), 40.0, 97, 61, step=0.5)
+    yield "ortho", W.ortho_lookat_camera(c + np.array([-1.7, 0.6, 1.1]) * max(n), c, (0, 1, 0), 1.6 * max(n), 80, 50, step=0.7)
+    yield "inside", W.perspective_camera((16.3, 7.25, 32.45), (30, 40, 10), (0, 0, 1), 70.0, 64, 48, step=0.5)
+    yield "axis", W.ortho_axis_camera(n, 0, -1, step=1.0)
+
+
+@pytest.mark.parametrize("ert", [0.0, 0.99])
+def test_single_march_views(ert):
+    n = (61, 47, 83)
+    v = W.make_cube(W.Recipe(*n, seed=31, n_sources=5))
+    s = O.minmax_hist(v)
+    R = float(max(abs(s.vmin), abs(s.vmax)))
+    tf = W.tf_opaque(n, 0.5) if ert else W.tf_haze(n, 0.5)
+    with vr.Volume(dev(v), n) as vol:
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for name, cam in _views(n):
+            cam = cam.with_(ert_alpha=ert)
+            om = O.render(v, cam, O.MIP)
+            check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)
+            oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
+            st = check_ea(vol.render(cam, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
+            if ert:
+                assert (oe.K_ert < oe.K).sum() > 20, name          # ERT really fires in this workload
+
+
+def test_all_miss_camera_and_eye_inside():
+    n = (20, 24, 28)
+    v = W.make_cube(W.Recipe(*n, seed=2))
+    cam = W.perspective_camera((100.0, 100.0, 100.0), (200, 200, 200), (0, 1, 0), 20.0, 33, 17)
+    with vr.Volume(dev(v), n) as vol:
+        vol.set_transfer_function(W.tf_haze(n, 0.5), -5.0, 5.0)
+        assert torch.isneginf(vol.render(cam, vr.VR_MIP)).all()
+        assert (vol.render(cam, vr.VR_EA) == 0).all()
+
+
+# ------------------------------------------------------------------ bricks: A0, A4, A10
+@pytest.mark.parametrize("B", [7, 16, 32, 100])
+def test_sort_last_equals_oracle_bricked(B):
+    n = (61, 47, 83)
+    v = W.make_cube(W.Recipe(*n, seed=33, n_sources=5))
+    s = O.minmax_hist(v)
+    R = float(max(abs(s.vmin), abs(s.vmax)))
+    tf = W.bake_tf(W.TF_HAZE_POINTS, 0.5, alpha_scale=6.0)
+    with vr.Volume(dev(v), n, brick=B) as vol:
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for name, cam in _views(n):
+            cam = cam.with_(flags=W.cameras.VR_SORT_LAST)
+            om = O.render(v, cam, O.MIP, brick=B)
+            assert om.n_noncontig == 0 and om.n_order_mismatch == 0
+            sm = check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)
+            assert sm["bit_exact"] == 1.0, name
+            oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax, brick=B)
+            se = check_ea(vol.render(cam, vr.VR_EA).cpu().numpy(), oe.image)
+            assert se["bit_exact"] == 1.0, (name, se)                # same partials, same fold order
+            st = vol.stats()
+            assert st["path"] == 2 and st["fragments"] > 0
+
+
+def test_sort_last_rejections():
+    n = (16, 16, 16)
+    v = W.make_cube(W.Recipe(*n, seed=1))
+    cam = W.ortho_axis_camera(n, 2, +1).with_(flags=W.cameras.VR_SORT_LAST)
+    with vr.Volume(dev(v), n, brick=0) as vol:
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cam, vr.VR_MIP)
+        assert e.value.status == vr.VR_ERR_UNSUPPORTED
+    with vr.Volume(dev(v), n, brick=8) as vol:
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cam, vr.VR_EA)
+        assert e.value.status == vr.VR_ERR_NOT_READY
+        vol.set_transfer_function(W.tf_haze(n, 0.5), -1.0, 1.0)
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cam.with_(ert_alpha=0.99), vr.VR_EA)
+        assert e.value.status == vr.VR_ERR_UNSUPPORTED
+
+
+# ------------------------------------------------------------------ bricked-halo layout, chain, out-of-core: A5
+@pytest.mark.parametrize("where", ["device", "host_resident", "host_ooc"])
+def test_bricked_halo_chain_and_streaming(where):
+    n = (61, 47, 83)
+    B = 16
+    v = W.make_cube(W.Recipe(*n, seed=35, n_sources=5))
+    t = W.retile_halo(v, B)
+    s = O.minmax_hist(v)
+    R = float(max(abs(s.vmin), abs(s.vmax)))
+    tf = W.tf_opaque(n, 0.5)
+    brick_bytes = (B + 1) ** 3 * 4
+    kw = {}
+    data = dev(t) if where == "device" else pinned(t)
+    if where == "host_ooc":
+        kw = dict(resident_bytes=11 * brick_bytes, n_copy_streams=4)     # 11 of 72 bricks fit
+    with vr.Volume(data, n, brick=B, layout=vr.VR_BRICKED_HALO1, **kw) as vol:
+        assert_summary_equal(gpu_summary(vol), s)
+        assert_summary_equal(gpu_summary(vol, 100, (-0.5, 2.0)), O.minmax_hist(v, 100, (-0.5, 2.0)))
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for name, cam in _views(n):
+            for ert in (0.0, 0.99):
+                cam2 = cam.with_(ert_alpha=ert)
+                om = O.render(v, cam2, O.MIP)
+                sm = check_mip(vol.render(cam2, vr.VR_MIP).cpu().numpy(), om.image, R)
+                assert sm["bit_exact"] == 1.0, name
+                oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax)
+                se = check_ea(vol.render(cam2, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
+                assert se["bit_exact"] == 1.0, (name, ert, se)           # chained state == single march
+        st = vol.stats()
+        assert st["path"] == 3
+        if where == "host_ooc":
+            assert st["h2d_bytes"] > 0 and st["resident_bytes"] == 11 * brick_bytes
+
+
+def test_host_linear_mirror_and_host_outputs():
+    n = (40, 36, 52)
+    v = W.make_cube(W.Recipe(*n, seed=37, n_sources=3))
+    s = O.minmax_hist(v)
+    tf = W.tf_haze(n, 0.5)
+    cam = W.orbit_camera(n, 1, 8, 96, 64, step=0.5, ert_alpha=0.99)
+    with vr.Volume(pinned(v), n, brick=16) as vol:
+        hbuf = torch.empty(32 + 8 * 256, dtype=torch.uint8).pin_memory()
+        vol.minmax_histogram(256, None, out=hbuf)
+        torch.cuda.synchronize()
+        assert_summary_equal(vr.Volume.read_summary(hbuf), s)
+        assert vol.stats()["h2d_bytes"] == v.nbytes
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        out = torch.empty((64, 96, 4), dtype=torch.float32).pin_memory()
+        vol.render(cam, vr.VR_EA, out=out)
+        torch.cuda.synchronize()
+        oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
+        check_ea(out.numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
+        assert vol.stats()["d2h_bytes"] == out.numel() * 4 and vol.stats()["h2d_bytes"] == 0
+
+
+def test_pageable_host_memory_is_rejected():
+    v = W.make_cube(W.Recipe(16, 16, 16, seed=1))
+    t = torch.from_numpy(v)                  # pageable
+    if (t.data_ptr() & 15) != 0:
+        pytest.skip("unaligned numpy buffer")
+    with pytest.raises(vr.VrError) as e:
+        vr.Volume(t, (16, 16, 16))
+    assert e.value.status == vr.VR_ERR_INVALID_ARG
+
+
+def test_two_handles_two_streams_and_pitch():
+    n = (32, 32, 32)
+    a = W.make_cube(W.Recipe(*n, seed=41))
+    b = W.make_cube(W.Recipe(*n, seed=42))
+    cam = W.orbit_camera(n, 0, 4, 70, 50, step=0.5)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with vr.Volume(dev(a), n) as va, vr.Volume(dev(b), n) as vb:
+        big = torch.zeros((50, 96), dtype=torch.float32, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s1):
+            ia = va.render(cam, vr.VR_MIP, out=big[:, :70], stream=s1)
+        with torch.cuda.stream(s2):
+            ib = vb.render(cam, vr.VR_MIP, stream=s2)
+        torch.cuda.synchronize()
+        assert np.array_equal(ia.cpu().numpy(), O.render(a, cam, O.MIP).image)
+        assert np.array_equal(ib.cpu().numpy(), O.render(b, cam, O.MIP).image)
+        assert (big[:, 70:] == 0).all()
