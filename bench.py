@@ -1,0 +1,391 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the hot path on B200, one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+A *step* is one pass of the whole hot path over one synthetic cube: the data-summary pass
+(vr_minmax_histogram: min/max, then the 256-bin histogram over [min,max]), vr_set_transfer_function
+with that range, and vr_render of every orbit view of the config (for cfg2: 16 perspective views,
+1024x1024, step 0.5, emission-absorption with early ray termination at alpha 0.99).
+
+value  = nominal voxel samples of all rendered views / step time, cube resident in HBM when the
+         timed region starts (CUDA events on the launching stream, max over ranks).
+e2e    = the same metric through the C ABI with HOST buffers: every step creates the handle on the
+         pinned host cube (1 GiB host->device inside the timed region), runs the same calls with
+         pinned host outputs (summary and images copied device->host) and destroys the handle.
+Multi-GPU: the path does not shard (north_star: one GPU, no collectives) => N independent replicas,
+"scaling": "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+ALU_SLOTS_PER_EA_SAMPLE = 64      # issue slots of one EA sample
+ALU_SLOTS_PER_MIP_SAMPLE = 45
+N_SM, LANES_PER_SM = 148, 128     # B200 (B200_PROFILING.md): 148 SMs, 4 x 32 fp32/int lanes each
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+# ---------------------------------------------------------------------------------- clocks
+_REASONS = {0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x10: "sync_boost",
+            0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown"}
+
+
+class ClockSampler(threading.Thread):
+    """Polls NVML for SM clock and clock-event reasons while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.1):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._halt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self._halt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    bits = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    bits = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for b, name in _REASONS.items():
+                    if bits & b:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._halt.wait(self.period)
+
+    def finish(self) -> dict:
+        self._halt.set()
+        if self.is_alive():
+            self.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml_unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def physical_gpu_index(local: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local])
+        except Exception:
+            return local
+    return local
+
+
+# ---------------------------------------------------------------------------------- workload
+def make_host_cube(cfg, pinned=True):
+    """The config's seeded cube in (pinned) host memory, filled in z-slabs by the shared generator."""
+    import torch
+    import workload as W
+    nx, ny, nz = cfg.dims
+    t = torch.empty((nz, ny, nx), dtype=torch.float32, pin_memory=pinned)
+    gen = W.CubeGenerator(cfg.recipe)
+    slab = max(1, (1 << 28) // (nx * ny))
+    for z0 in range(0, nz, slab):
+        z1 = min(nz, z0 + slab)
+        gen.fill_ptr(t.data_ptr() + 4 * z0 * ny * nx, z0, z1)
+    return t
+
+
+def modes_of(cfg):
+    import paper_1111_6661_b200 as vr
+    return [vr.VR_EA if m == "ea" else vr.VR_MIP for m in cfg.modes]
+
+
+# ---------------------------------------------------------------------------------- reference arm
+def cpu_oracle_rate(cfg, host_np, tf, vmin, vmax, budget_s=15.0, view=0):
+    """Times the oracle as it stands (f32-canonical, OpenMP on all host cores) on a pixel lattice of
+    one view of the workload; returns samples/s and what the sample was."""
+    import oracle as O
+    cam = cfg.camera(view)
+    H, Wd = cam.height, cam.width
+    mode = O.EA if "ea" in cfg.modes else O.MIP
+
+    def run(stride):
+        mask = np.zeros((H, Wd), dtype=np.uint8)
+        mask[stride // 2::stride, stride // 2::stride] = 1
+        t0 = time.perf_counter()
+        r = O.render(host_np, cam, mode, tf, vmin, vmax, mask=mask)
+        dt = time.perf_counter() - t0
+        n = r.n_ert if mode == O.EA else r.n_nominal
+        return r.n_nominal, n, dt
+
+    n_nom, n_done, dt = run(16)                       # calibration pass
+    rate = max(n_nom / max(dt, 1e-6), 1.0)
+    total = n_nom * 256.0
+    stride = int(np.clip(np.ceil(np.sqrt(total / (rate * budget_s))), 1, 16))
+    if stride < 16:
+        n_nom, n_done, dt = run(stride)
+    return {"value": n_nom / dt, "unit": "samples/s", "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"{cfg.name} view {view}, every {stride}th pixel in x and y ({n_nom} nominal samples, "
+                      f"{n_done} evaluated before ERT, {dt:.2f} s), f32-canonical oracle, OpenMP",
+            "seconds": dt, "n_samples": int(n_nom)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import workload as W
+    import oracle as O
+    cfg = W.get_config(args.config)
+    host = make_host_cube(cfg, pinned=False).numpy()
+    s = O.minmax_hist(host[: max(2, min(host.shape[0], (1 << 27) // (host.shape[1] * host.shape[2])))])
+    tf = W.tf_haze(cfg.dims, cfg.step)
+    budget = 45.0 / max(args.steps + args.warmup, 1)
+    times, n = [], 0
+    for it in range(args.warmup + args.steps):
+        r = cpu_oracle_rate(cfg, host, tf, float(s.vmin), float(s.vmax), budget_s=min(budget, 15.0),
+                            view=it % cfg.n_views)
+        if it >= args.warmup:
+            times.append(r["seconds"]); n += r["n_samples"]
+    value = n / sum(times)
+    line = {"impl": "reference", "metric": "voxel_samples_per_s", "value": value, "unit": "samples/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * sum(times) / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": config_block(cfg, "bounded sample per step: one orbit view on a pixel lattice"),
+            "cpu_baseline": {"value": value, "unit": "samples/s", "cores": O.num_threads(), "kind": "oracle",
+                             "sample": r["sample"]},
+            "e2e": {"value": value, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def config_block(cfg, note=""):
+    nx, ny, nz = cfg.dims
+    return {"workload": f"{cfg.name}: {nx}x{ny}x{nz} float32 noise+{cfg.recipe.n_sources} sources, "
+                        f"{cfg.n_views} orbit views {cfg.width}x{cfg.height}, step {cfg.step}, "
+                        f"modes {'+'.join(cfg.modes)}, ERT {cfg.ert_alpha}, TF_HAZE, + min/max & 256-bin histogram",
+            "cube_bytes": 4 * nx * ny * nz, "brick": cfg.brick, "views": cfg.n_views,
+            "image": [cfg.width, cfg.height], "l2": "inputs larger than L2 (cube >= 1 GiB, orbit views evict each other)",
+            "parallelism": "replicas", "note": note}
+
+
+# ---------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import paper_1111_6661_b200 as vr
+    import workload as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = W.get_config(args.config)
+    nx, ny, nz = cfg.dims
+    n_vox = nx * ny * nz
+    host = make_host_cube(cfg, pinned=True)
+    dev = host.cuda()
+    stream = torch.cuda.current_stream()
+    modes = modes_of(cfg)
+    cams = [cfg.camera(v) for v in range(cfg.n_views)]
+    cam_structs = [vr.make_camera(c) for c in cams]
+    samples_view = [W.nominal_samples(c, cfg.dims) for c in cams]
+    samples_step = sum(samples_view) * len(modes)
+    frames_step = len(cams) * len(modes)
+
+    vol = vr.Volume(dev, cfg.dims, brick=cfg.brick)
+    sbuf = torch.empty(32 + 8 * 256, dtype=torch.uint8, device="cuda")
+    s = vr.Volume.read_summary(vol.minmax_histogram(256, out=sbuf))
+    vmin, vmax = float(s["vmin"]), float(s["vmax"])
+    tf = W.tf_haze(cfg.dims, cfg.step)
+    images = {m: torch.empty((cfg.height, cfg.width, 4) if m == vr.VR_EA else (cfg.height, cfg.width),
+                             dtype=torch.float32, device="cuda") for m in modes}
+
+    ev_pairs = []                                    # (start, end) around every vr_render of the timed region
+
+    def step(record=False):
+        vol.minmax_histogram(256, out=sbuf)
+        vol.set_transfer_function(tf, vmin, vmax)
+        n = 0
+        for m in modes:
+            for c in cam_structs:
+                if record:
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                vol.render(c, m, out=images[m])
+                if record:
+                    b.record(stream); ev_pairs.append((a, b))
+                n += vol.stats()["kernel_launches"]
+        return n
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    clocks = ClockSampler(physical_gpu_index(local))
+    clocks.start()
+    launches0 = vol.stats()["total_kernel_launches"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step(record=True)
+    e1.record(stream)
+    barrier()
+    clk = clocks.finish()
+    ms_total = e0.elapsed_time(e1)
+    launches = vol.stats()["total_kernel_launches"] - launches0
+    render_ms = [a.elapsed_time(b) for a, b in ev_pairs]
+    path = vol.stats()["path"]
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * samples_step / (ms_step * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers (every step uploads the cube)
+    h_sum = torch.empty(32 + 8 * 256, dtype=torch.uint8).pin_memory()
+    h_img = {m: torch.empty(tuple(images[m].shape), dtype=torch.float32).pin_memory() for m in modes}
+
+    def e2e_step():
+        with vr.Volume(host, cfg.dims, brick=cfg.brick, n_copy_streams=4) as hv:
+            hv.minmax_histogram(256, out=h_sum)
+            h2d = hv.stats()["h2d_bytes"]
+            torch.cuda.current_stream().synchronize()
+            hs = vr.Volume.read_summary(h_sum)
+            hv.set_transfer_function(tf, float(hs["vmin"]), float(hs["vmax"]))
+            d2h = 32 + 8 * 256
+            for m in modes:
+                for c in cam_structs:
+                    hv.render(c, m, out=h_img[m])
+                    d2h += hv.stats()["d2h_bytes"]
+            torch.cuda.current_stream().synchronize()
+        return h2d, d2h
+
+    vol.close()
+    del dev
+    torch.cuda.empty_cache()
+    e2e_steps = max(1, min(args.steps, 3))
+    e2e_step()
+    barrier()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(e2e_steps):
+        h2d, d2h = e2e_step()
+    b.record(stream)
+    barrier()
+    e2e_ms = a.elapsed_time(b)
+    if dist is not None:
+        t = torch.tensor([e2e_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = world * samples_step / (e2e_ms / e2e_steps * 1e-3)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the ray-march kernel: one launch per vr_render on path 1)
+    hbm_peak, sm_max_mhz, peak_src = measured_peaks()
+    k_ms = float(np.mean(render_ms))
+    ea_frac = sum(1 for m in modes if m == vr.VR_EA) / len(modes)
+    slots = ALU_SLOTS_PER_EA_SAMPLE * ea_frac + ALU_SLOTS_PER_MIP_SAMPLE * (1 - ea_frac)
+    samples_launch = float(np.mean(samples_view))
+    bytes_launch = 4.0 * n_vox + 4.0 * cfg.width * cfg.height * (4 * ea_frac + (1 - ea_frac))
+    alu_peak = N_SM * LANES_PER_SM * sm_max_mhz * 1e6              # lane-instructions / s
+    hbm_floor_ms = bytes_launch / (hbm_peak * 1e9) * 1e3
+    alu_floor_ms = slots * samples_launch / alu_peak * 1e3
+    hbm_roof = {"bound": "hbm", "achieved": bytes_launch / (k_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "traffic": None, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
+                "algorithmic_bytes_per_launch": bytes_launch, "floor_ms": hbm_floor_ms}
+    hbm_roof["frac"] = hbm_roof["achieved"] / hbm_peak
+    alu_roof = {"bound": "alu", "achieved": slots * samples_launch / (k_ms * 1e-3) / 1e12, "peak": alu_peak / 1e12,
+                "unit": "Tlane-instr/s", "traffic": None,
+                "peak_source": f"{N_SM} SMs x {LANES_PER_SM} lanes x {sm_max_mhz:.0f} MHz (DESIGN.md §6)",
+                "algorithmic_slots_per_sample": slots, "floor_ms": alu_floor_ms}
+    alu_roof["frac"] = alu_roof["achieved"] / alu_roof["peak"]
+    primary, other = (alu_roof, hbm_roof) if alu_floor_ms > hbm_floor_ms else (hbm_roof, alu_roof)
+    primary = dict(primary, kernel="k_march (vr_render, single-march path)" if path == 1 else f"vr_render path {path}",
+                   kernel_ms=k_ms, launches_timed=len(render_ms))
+
+    line = {"metric": "voxel_samples_per_s", "value": value, "unit": "samples/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": config_block(cfg), "clocks": clk,
+            "e2e": {"value": e2e_value, "unit": "samples/s", "h2d_bytes_per_step": int(h2d),
+                    "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps},
+            "gpu_launches": int(launches),
+            "roofline": primary, "roofline_other": other,
+            "frames_per_s": world * frames_step / (ms_step * 1e-3),
+            "render_ms": {"min": float(np.min(render_ms)), "median": float(np.median(render_ms)),
+                          "mean": k_ms, "max": float(np.max(render_ms))},
+            "render_share_of_step": float(np.sum(render_ms)) / ms_total,
+            "effective_hbm_gbs_per_frame": 4.0 * n_vox / (k_ms * 1e-3) / 1e9,
+            "samples_per_step": int(samples_step)}
+    if world == 1 and not args.no_cpu:
+        line["cpu_baseline"] = cpu_oracle_rate(cfg, host.numpy(), tf, vmin, vmax, budget_s=args.cpu_seconds)
+    else:
+        line["cpu_baseline"] = None
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (default 2 = configs[1])")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

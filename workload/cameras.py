@@ -121,3 +121,30 @@ def orbit_camera(dims, view: int, n_views: int, width: int, height: int, step: f
     cam = perspective_camera(eye, c, (0.0, 1.0, 0.0), fov_y_deg, width, height, step=step, **kw)
     cam.meta.update({"kind": "orbit", "view": view, "n_views": n_views, "R": R})
     return cam
+
+
+def nominal_samples(cam: Camera, dims) -> int:
+    """Size of one view as a workload: how many sample positions its rays hold inside the box
+    [0,nx]x[0,ny]x[0,nz] at spacing ``cam.step`` (mid-point lattice from the volume entry), counted
+    analytically in float64 from the camera geometry.  A descriptor of the input (like a token
+    count), used by bench.py to turn frame times into samples/s; it may differ from the renderer's
+    own float32 count by at most one sample per ray."""
+    v = cam.vectors().astype(np.float64)
+    W, H = cam.width, cam.height
+    px = (np.arange(W, dtype=np.float64) + 0.5)[None, :, None]
+    py = (np.arange(H, dtype=np.float64) + 0.5)[:, None, None]
+    o = v[0] + px * v[1] + py * v[2]
+    g = v[3] + px * v[4] + py * v[5]
+    d = g / np.linalg.norm(g, axis=-1, keepdims=True)
+    n = np.asarray(dims, dtype=np.float64)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        ta, tb = (0.0 - o) / d, (n - o) / d
+    lo, hi = np.minimum(ta, tb), np.maximum(ta, tb)
+    par = d == 0.0
+    inside = (o >= 0.0) & (o <= n)
+    lo = np.where(par, np.where(inside, -np.inf, np.inf), lo)
+    hi = np.where(par, np.where(inside, np.inf, -np.inf), hi)
+    t_enter = np.maximum(lo.max(axis=-1), 0.0)
+    t_exit = hi.min(axis=-1)
+    chord = np.where(t_exit > t_enter, t_exit - t_enter, 0.0)
+    return int(np.maximum(np.ceil(chord / float(cam.step) - 0.5), 0.0).sum())
