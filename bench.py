@@ -305,15 +305,18 @@ def run_ours(args):
     del dev
     torch.cuda.empty_cache()
     e2e_steps = max(1, min(args.steps, 3))
-    e2e_step()
-    barrier()
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record(stream)
-    for _ in range(e2e_steps):
-        h2d, d2h = e2e_step()
-    b.record(stream)
-    barrier()
-    e2e_ms = a.elapsed_time(b)
+    h2d = d2h = 0
+    e2e_ms = float("nan")
+    if not args.no_e2e:
+        e2e_step()
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(e2e_steps):
+            h2d, d2h = e2e_step()
+        b.record(stream)
+        barrier()
+        e2e_ms = a.elapsed_time(b)
     if dist is not None:
         t = torch.tensor([e2e_ms], device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -379,6 +382,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (default 2 = configs[1])")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     if args.impl == "reference":

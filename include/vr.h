@@ -204,7 +204,7 @@ typedef struct {
     uint32_t n_bricks;              /* bricks in the grid */
     uint32_t bricks_drawn;          /* bricks that produced work in the last render */
     uint32_t bricks_culled;         /* bricks outside the view (empty screen rectangle) */
-    uint32_t path;                  /* last render: 0 none, 1 single march, 2 sort-last, 3 streamed chain */
+    uint32_t path;                  /* last render: 0 none, 1 ray-major march, 2 sort-last, 3 brick chain, 4 tile-wave */
     uint32_t kernel_launches;       /* library kernels launched by the last call */
     uint64_t fragments;             /* (brick,pixel) partial fragments written (sort-last) */
     uint64_t h2d_bytes;             /* host-to-device bytes enqueued by the last call */
@@ -214,6 +214,21 @@ typedef struct {
 } vr_stats;
 
 VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
+
+/* ------------------------------------------------------------------------------------------
+ * vr_set_option — implementation choices that never change results beyond the documented
+ * tolerances (all paths evaluate the same canonical arithmetic, C.1-C.7); used by the parity
+ * tests to force each path and by bench.py for ablations.
+ *   VR_OPT_RENDER_PATH  how a device-resident VR_LINEAR volume is marched when VR_SORT_LAST is
+ *                       not requested: 0 = auto (tile-wave when the camera is purely perspective
+ *                       or purely orthographic), 1 = ray-major (one thread per ray through
+ *                       global memory), 2 = tile-wave (falls back to ray-major for mixed cameras).
+ *   VR_OPT_TILE_SHAPE   staging tile of the tile-wave path: 0 = auto, 1 = 32x32x32,
+ *                       2 = 32x32x16, 3 = 32x16x16, 4 = 16x16x16 ownership cells.
+ * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).
+ * ------------------------------------------------------------------------------------------ */
+enum { VR_OPT_RENDER_PATH = 1, VR_OPT_TILE_SHAPE = 2 };
+VR_API vr_status vr_set_option(vr_volume *vol, uint32_t option, int64_t value);
 
 /* Thread-local message of the last failing call on this thread ("" if none). */
 VR_API const char *vr_last_error(void);

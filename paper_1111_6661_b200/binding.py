@@ -18,6 +18,8 @@ VR_LINEAR, VR_BRICKED_HALO1 = 0, 1
 VR_DEVICE, VR_HOST_PINNED = 0, 1
 VR_EA, VR_MIP = 0, 1
 VR_SORT_LAST = 1
+VR_OPT_RENDER_PATH, VR_OPT_TILE_SHAPE = 1, 2
+VR_PATH_AUTO, VR_PATH_RAY_MAJOR, VR_PATH_TILE_WAVE = 0, 1, 2
 
 _STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_UNSUPPORTED", 3: "VR_ERR_OUT_OF_MEMORY",
            4: "VR_ERR_CUDA", 5: "VR_ERR_NOT_READY"}
@@ -55,7 +57,7 @@ class vr_stats(C.Structure):
 
 
 EXPORTS = ("vr_create_volume", "vr_destroy_volume", "vr_set_transfer_function", "vr_render",
-           "vr_minmax_histogram", "vr_get_stats", "vr_last_error", "vr_version")
+           "vr_minmax_histogram", "vr_get_stats", "vr_set_option", "vr_last_error", "vr_version")
 
 _lib = None
 
@@ -82,6 +84,8 @@ def load():
         lib.vr_minmax_histogram.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
         lib.vr_get_stats.restype = C.c_int
         lib.vr_get_stats.argtypes = [C.c_void_p, C.POINTER(vr_stats)]
+        lib.vr_set_option.restype = C.c_int
+        lib.vr_set_option.argtypes = [C.c_void_p, C.c_uint32, C.c_int64]
         lib.vr_last_error.restype = C.c_char_p
         lib.vr_version.restype = C.c_char_p
         _lib = lib
@@ -211,6 +215,10 @@ class Volume:
             torch.cuda.current_stream().synchronize()
             buf = buf.cpu()
         return np.frombuffer(buf.numpy().tobytes()[: 32 + 8 * nbins], dtype=summary_dtype(nbins))[0]
+
+    # -- vr_set_option
+    def set_option(self, option: int, value: int):
+        _check(load().vr_set_option(self._h, int(option), int(value)))
 
     # -- vr_get_stats
     def stats(self) -> dict:

@@ -97,6 +97,13 @@ struct vr_volume {
     SummaryScratch *d_sum = nullptr;
     vr_summary *d_sum_out = nullptr;          // staging for host outputs
     DevBuf<float> arena, host_image;
+
+    // tile-wave path
+    DevBuf<unsigned char> tile_work;
+    DevBuf<unsigned int> tile_ctrl, tile_done;
+    unsigned int tile_serial = 0;
+    uint64_t tile_done_sig = 0;               // tile grid the done flags were cleared for
+    int opt_path = 0, opt_tile = 0;           // vr_set_option
     Staging staging[kStagingRing];
     int staging_next = 0;
 
@@ -125,6 +132,7 @@ static void free_volume(vr_volume *v)
     if (v->d_sum_out) cudaFree(v->d_sum_out);
     v->arena.release();
     v->host_image.release();
+    v->tile_work.release(); v->tile_ctrl.release(); v->tile_done.release();
     delete v;
 }
 
@@ -445,6 +453,97 @@ static vr_status render_chain(vr_volume *v, const vr_camera *c, const CamK &cam,
     return VR_OK;
 }
 
+// tile-wave march of a device-resident linear volume (vr_tiles.cu): exact ERT, one pass over the voxels
+static bool tiles_applicable(const vr_volume *v, const vr_camera *c, bool persp, bool ortho)
+{
+    if (v->opt_path == 1) return false;
+    if (v->desc.layout != VR_LINEAR || v->out_of_core || !(persp || ortho)) return false;
+    (void)c;
+    return true;
+}
+
+static vr_status render_tiles(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, bool persp,
+                              const TfK &tf, float *img, long long pitch_f, cudaStream_t st)
+{
+    const int n[3] = { (int)v->desc.nx, (int)v->desc.ny, (int)v->desc.nz };
+    int kind = v->opt_tile;
+    if (kind <= 0 || kind >= VR_TILE_KINDS) kind = VR_TILE_32x32x16;
+    TilePlanK P;
+    tile_dims(kind, P.T);
+    P.persp = persp ? 1 : 0;
+    long long n_tiles = 1;
+    int max_lvl[3];
+    for (int a = 0; a < 3; ++a) {
+        P.nt[a] = std::max(1, (n[a] - 1 + P.T[a] - 1) / P.T[a]);       // base indices 0 .. n-2
+        n_tiles *= P.nt[a];
+        const float oc = c->o0[a] - 0.5f;                              // float32, as make_ray forms it (C.3)
+        const double fl = std::floor((double)oc);
+        const long long fi = (long long)std::min(std::max(fl, -1e15), 1e15);
+        long long e = fi >= 0 ? fi / P.T[a] : -((-fi + P.T[a] - 1) / P.T[a]);
+        e = std::min<long long>(std::max<long long>(e, -(1 << 28)), 1 << 28);
+        P.e[a] = (int)e;
+        P.sgn[a] = c->d0[a] > 0.0f ? 1 : c->d0[a] < 0.0f ? -1 : 0;
+        P.lvl0[a] = 0;
+        if (persp) {
+            P.lvl0[a] = P.e[a] < 0 ? -P.e[a] : P.e[a] > P.nt[a] - 1 ? P.e[a] - (P.nt[a] - 1) : 0;
+            max_lvl[a] = std::max(tile_axis_level(P, a, 0), tile_axis_level(P, a, P.nt[a] - 1));
+        } else max_lvl[a] = P.sgn[a] ? P.nt[a] - 1 : 0;
+    }
+    if (n_tiles > 0x3fffffffll || P.nt[0] > 65535 || P.nt[1] > 65535 || P.nt[2] > 65535) {
+        set_error("tile grid too large"); return VR_ERR_UNSUPPORTED;
+    }
+    P.n_tiles = (int)n_tiles;
+    P.n_levels = max_lvl[0] + max_lvl[1] + max_lvl[2] + 1;
+
+    // tiles per level = convolution of the three per-axis level histograms
+    std::vector<unsigned long long> hx(max_lvl[0] + 1, 0), hy(max_lvl[1] + 1, 0), hz(max_lvl[2] + 1, 0), hxy(max_lvl[0] + max_lvl[1] + 1, 0);
+    for (int b = 0; b < P.nt[0]; ++b) hx[tile_axis_level(P, 0, b)]++;
+    for (int b = 0; b < P.nt[1]; ++b) hy[tile_axis_level(P, 1, b)]++;
+    for (int b = 0; b < P.nt[2]; ++b) hz[tile_axis_level(P, 2, b)]++;
+    for (size_t i = 0; i < hx.size(); ++i) for (size_t j = 0; j < hy.size(); ++j) hxy[i + j] += hx[i] * hy[j];
+    std::vector<unsigned long long> cnt(P.n_levels, 0);
+    for (size_t i = 0; i < hxy.size(); ++i) if (hxy[i]) for (size_t j = 0; j < hz.size(); ++j) cnt[i + j] += hxy[i] * hz[j];
+
+    Staging *s;
+    vr_status rc = staging_acquire(v, (size_t)(P.n_levels + 1) * sizeof(unsigned int), &s);
+    if (rc != VR_OK) return rc;
+    unsigned int *off = reinterpret_cast<unsigned int *>(s->h);
+    unsigned long long acc = 0;
+    for (int l = 0; l < P.n_levels; ++l) { off[l] = (unsigned int)acc; acc += cnt[l]; }
+    off[P.n_levels] = (unsigned int)acc;
+    if (acc != (unsigned long long)n_tiles) { set_error("internal: tile level counts do not add up"); return VR_ERR_UNSUPPORTED; }
+
+    if ((rc = v->tile_work.reserve((size_t)n_tiles * sizeof(TileWork))) != VR_OK) return rc;
+    if ((rc = v->tile_ctrl.reserve((size_t)P.n_levels + 1)) != VR_OK) return rc;
+    const uint64_t sig = ((uint64_t)kind << 32) | (uint64_t)n_tiles;
+    if (v->tile_done.cap < (size_t)n_tiles || sig != v->tile_done_sig) {
+        if ((rc = v->tile_done.reserve((size_t)n_tiles)) != VR_OK) return rc;
+        VR_CUDA(cudaMemsetAsync(v->tile_done.p, 0, v->tile_done.cap * sizeof(unsigned int), st));
+        v->tile_done_sig = sig;
+    }
+    const unsigned int serial = ++v->tile_serial;
+
+    VolK V;
+    V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
+    V.nx = n[0]; V.ny = n[1]; V.nz = n[2]; V.ox = V.oy = V.oz = 0;
+    VR_CUDA(cudaMemsetAsync(v->tile_ctrl.p, 0, ((size_t)P.n_levels + 1) * sizeof(unsigned int), st));
+    VR_CUDA(cudaMemcpyAsync(s->d, s->h, (size_t)(P.n_levels + 1) * sizeof(unsigned int), cudaMemcpyHostToDevice, st));
+    v->stats.h2d_bytes += (size_t)(P.n_levels + 1) * sizeof(unsigned int);
+    launch_tile_plan(cam, P, V, reinterpret_cast<const unsigned int *>(s->d), v->tile_ctrl.p,
+                     reinterpret_cast<TileWork *>(v->tile_work.p), st);
+    launch_chain_init(mode, cam.width, cam.height, img, pitch_f, st);
+    rc = launch_tile_march(kind, mode, ert, cam, P, V, tf, reinterpret_cast<const TileWork *>(v->tile_work.p),
+                           v->tile_ctrl.p, v->tile_done.p, serial, img, pitch_f, v->sm_count, st);
+    if (rc != VR_OK) return rc;
+    v->stats.kernel_launches += 3;
+    if (mode == VR_EA) { launch_chain_finish(cam.width, cam.height, img, pitch_f, st); v->stats.kernel_launches += 1; }
+    VR_CUDA(cudaEventRecord(s->done, st));
+    s->in_flight = true;
+    v->stats.path = 4;
+    v->stats.bricks_drawn = (uint32_t)n_tiles;
+    return VR_OK;
+}
+
 }  // namespace vr
 
 // ====================================================================== C ABI
@@ -618,6 +717,7 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     TfK tf; tf.table = v->d_tf; tf.scale = v->tf_scale; tf.bias = v->tf_bias;
     if (sort_last) rc = render_sort_last(v, c, cam, mode, tf, img, pitch_f, st);
     else if (v->out_of_core || v->desc.layout == VR_BRICKED_HALO1) rc = render_chain(v, c, cam, mode, ert, tf, img, pitch_f, st);
+    else if (tiles_applicable(v, c, persp, ortho)) rc = render_tiles(v, c, cam, mode, ert, persp, tf, img, pitch_f, st);
     else rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
     if (rc != VR_OK) return rc;
     VR_CUDA(cudaGetLastError());
@@ -700,6 +800,22 @@ VR_API vr_status vr_minmax_histogram(vr_volume *v, uint32_t nbins, const float *
     VR_CUDA(cudaGetLastError());
     v->stats.total_kernel_launches += v->stats.kernel_launches;
     return VR_OK;
+}
+
+VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
+{
+    g_err[0] = 0;
+    VR_REQUIRE(v, "vr_set_option: NULL handle");
+    switch (option) {
+    case VR_OPT_RENDER_PATH:
+        VR_REQUIRE(value >= 0 && value <= 2, "VR_OPT_RENDER_PATH: 0 auto, 1 ray-major, 2 tile-wave (got %lld)", (long long)value);
+        v->opt_path = (int)value; return VR_OK;
+    case VR_OPT_TILE_SHAPE:
+        VR_REQUIRE(value >= 0 && value < VR_TILE_KINDS, "VR_OPT_TILE_SHAPE: 0..%d (got %lld)", VR_TILE_KINDS - 1, (long long)value);
+        v->opt_tile = (int)value; return VR_OK;
+    default:
+        set_error("unknown option %u", option); return VR_ERR_INVALID_ARG;
+    }
 }
 
 VR_API vr_status vr_get_stats(vr_volume *v, vr_stats *s)

@@ -81,4 +81,49 @@ void launch_chain_brick(int mode, bool ert, const CamK &cam, const VolK &vol, co
                         float *image, long long pitch_f, cudaStream_t st);
 void launch_chain_finish(int W, int H, float *image, long long pitch_f, cudaStream_t st);
 
+// ---------------------------------------------------------------- tile-wave ray casting (vr_tiles.cu)
+// The volume is cut into staging tiles of TX x TY x TZ ownership cells (a finer brick grid, C.7).
+// A persistent kernel stages one tile at a time in shared memory and marches every ray segment
+// that crosses it; tiles are taken front to back (level = per-axis tile distance from the eye
+// tile) and a tile starts once its <= 3 face neighbours towards the eye are complete, so the ray
+// state carried in the image sees its samples in k order (exact C.5 / ERT).
+struct TileWork {                // one entry of the per-frame work list (level-major)
+    int x0, y0, x1, y1;          // conservative screen rectangle, [x0,x1) x [y0,y1); empty => no work
+    unsigned short b[3];         // tile coordinates
+    unsigned short flags;
+};
+
+struct TilePlanK {
+    int nt[3];                   // tiles per axis
+    int T[3];                    // tile edge per axis
+    int persp;                   // 1: pure perspective (ou = ov = 0); 0: pure orthographic (du = dv = 0)
+    int e[3];                    // perspective: tile index of the eye, floor(floor(o0 - 0.5) / T), unclamped
+    int sgn[3];                  // orthographic: sign of d0 per axis
+    int lvl0[3];                 // per-axis minimum raw level (subtracted so that levels start at 0)
+    int n_tiles, n_levels;
+};
+
+__host__ __device__ inline int tile_axis_level(const TilePlanK &P, int a, int b)
+{
+    if (P.persp) return (b > P.e[a] ? b - P.e[a] : P.e[a] - b) - P.lvl0[a];
+    return P.sgn[a] > 0 ? b : P.sgn[a] < 0 ? P.nt[a] - 1 - b : 0;
+}
+// tile coordinate of the face neighbour towards the eye on axis a, or -1
+__host__ __device__ inline int tile_axis_pred(const TilePlanK &P, int a, int b)
+{
+    int p;
+    if (P.persp) p = b > P.e[a] ? b - 1 : b < P.e[a] ? b + 1 : -1;
+    else p = P.sgn[a] > 0 ? b - 1 : P.sgn[a] < 0 ? b + 1 : -1;
+    return (p < 0 || p >= P.nt[a]) ? -1 : p;
+}
+
+enum { VR_TILE_32 = 1, VR_TILE_32x32x16 = 2, VR_TILE_32x16x16 = 3, VR_TILE_16 = 4, VR_TILE_KINDS = 5 };
+void tile_dims(int kind, int T[3]);
+// ctrl: [0] pop counter, [1 .. n_levels] per-level fill cursors (zeroed before each frame)
+void launch_tile_plan(const CamK &cam, const TilePlanK &P, const VolK &vol, const unsigned int *lvl_off,
+                      unsigned int *ctrl, TileWork *work, cudaStream_t st);
+vr_status launch_tile_march(int kind, int mode, bool ert, const CamK &cam, const TilePlanK &P, const VolK &vol,
+                            const TfK &tf, const TileWork *work, unsigned int *ctrl, unsigned int *done,
+                            unsigned int serial, float *image, long long pitch_f, int sm_count, cudaStream_t st);
+
 }  // namespace vr

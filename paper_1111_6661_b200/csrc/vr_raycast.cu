@@ -10,6 +10,7 @@
 // the slab of the volume the active tiles are crossing).  The 256-entry RGBA transfer function
 // lives in shared memory (4 KiB + one pad entry).
 #include "vr_internal.h"
+#include "vr_range.cuh"
 
 namespace vr {
 
@@ -94,60 +95,11 @@ k_march_full(CamK cam, VolK V, TfK tf, float *__restrict__ image, long long pitc
             make_float4(A.cr, A.cg, A.cb, __fsub_rn(1.0f, A.T));
 }
 
-// ---------------------------------------------------------------- per-(ray, brick) sample range
-// C.7: sample k is owned by the brick iff its clamped base index i0 lies in [lo, hi] on every
-// axis.  i0_a(k) is monotone in k, so the owned samples form one contiguous k-range.  It is
-// estimated from the slab interval of the ownership cell and then FIXED UP by evaluating the
-// exact predicate at the ends, so every sample has exactly one owner whatever the rounding.
-__device__ __forceinline__ bool owned(const VolK &V, const Ray &r, float step, const BrickK &b, int k)
-{
-    if (k < 0) return false;
-    const float t = __fmaf_rn((float)k, step, r.t_first);
-    if (!(t < r.t_exit)) return false;
-    int i; float f;
-    axis_cell(t, r.d[0], r.oc[0], V.nx, i, f);
-    if (i < b.lo[0] || i > b.hi[0]) return false;
-    axis_cell(t, r.d[1], r.oc[1], V.ny, i, f);
-    if (i < b.lo[1] || i > b.hi[1]) return false;
-    axis_cell(t, r.d[2], r.oc[2], V.nz, i, f);
-    return i >= b.lo[2] && i <= b.hi[2];
-}
-
+// per-(ray, brick) sample range: box_range() of vr_range.cuh
 __device__ __forceinline__ bool brick_range(const VolK &V, const Ray &r, float step, const BrickK &b, int &k_lo,
                                             int &k_hi)
 {
-    const int n[3] = { V.nx, V.ny, V.nz };
-    float t_lo = r.t_first, t_hi = r.t_exit;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const float qlo = b.lo[a] == 0 ? -CUDART_INF_F : (float)b.lo[a];
-        const float qhi = b.hi[a] == n[a] - 2 ? CUDART_INF_F : (float)(b.hi[a] + 1);
-        if (r.d[a] != 0.0f) {
-            const float inv = __fdividef(1.0f, r.d[a]);
-            const float t0 = (qlo - r.oc[a]) * inv, t1 = (qhi - r.oc[a]) * inv;
-            t_lo = fmaxf(t_lo, fminf(t0, t1));
-            t_hi = fminf(t_hi, fmaxf(t0, t1));
-        } else {
-            int i; float f;
-            axis_cell(0.0f, 0.0f, r.oc[a], n[a], i, f);          // q == oc for every sample
-            if (i < b.lo[a] || i > b.hi[a]) return false;
-        }
-    }
-    const float inv_step = __fdividef(1.0f, step);
-    const float pad_f = fminf(2.0f + 8e-6f * fabsf(r.t_exit) * inv_step, 64.0f);   // rounding slack of the estimate
-    const float a_f = (t_lo - r.t_first) * inv_step, b_f = (t_hi - r.t_first) * inv_step;
-    if (!(b_f + pad_f >= a_f - pad_f)) return false;
-    const int pad = (int)pad_f;
-    int kl = (int)fminf(fmaxf(ceilf(a_f), 0.0f), 16777216.0f) - pad;
-    int kh = (int)fminf(fmaxf(floorf(b_f), -1.0f), 16777216.0f) + pad;
-    kl = max(kl, 0);
-    while (kl <= kh && !owned(V, r, step, b, kl)) ++kl;
-    if (kl > kh) return false;
-    while (owned(V, r, step, b, kl - 1)) --kl;
-    while (kh > kl && !owned(V, r, step, b, kh)) --kh;
-    while (owned(V, r, step, b, kh + 1)) ++kh;
-    k_lo = kl; k_hi = kh;
-    return true;
+    return box_range(V.nx, V.ny, V.nz, r, step, b.lo, b.hi, k_lo, k_hi);
 }
 
 // ---------------------------------------------------------------- per-brick partial images

@@ -77,6 +77,10 @@ def test_cfg1_full():
         ea = vol.render(cam, vr.VR_EA).cpu().numpy()
         ea2 = vol.render(cam, vr.VR_EA).cpu().numpy()
         st = vol.stats()
+        vol.set_option(vr.VR_OPT_RENDER_PATH, vr.VR_PATH_RAY_MAJOR)
+        mip_r = vol.render(cam, vr.VR_MIP).cpu().numpy()
+        ea_r = vol.render(cam, vr.VR_EA).cpu().numpy()
+        st_r = vol.stats()
     R = float(max(abs(o_sum.vmin), abs(o_sum.vmax)))
     om = O.render(v, cam, O.MIP)
     oe = O.render(v, cam, O.EA, tf, o_sum.vmin, o_sum.vmax)
@@ -84,7 +88,9 @@ def test_cfg1_full():
     se = check_ea(ea, oe.image)
     assert sm["bit_exact"] == 1.0 and se["bit_exact"] == 1.0        # same canonical op sequence
     assert np.array_equal(ea, ea2)                                   # run-to-run determinism
-    assert st["path"] == 1 and st["kernel_launches"] == 1
+    assert st["path"] == 4                                           # auto = tile-wave for a pure ortho camera
+    assert st_r["path"] == 1 and st_r["kernel_launches"] == 1
+    assert check_mip(mip_r, om.image, R)["bit_exact"] == 1.0 and check_ea(ea_r, oe.image)["bit_exact"] == 1.0
 
 
 def _views(n):
@@ -95,23 +101,65 @@ def _views(n):
     yield "axis", W.ortho_axis_camera(n, 0, -1, step=1.0)
 
 
+# path 1 = ray-major through global memory; path 2 = tile-wave with each staging-tile shape
+@pytest.mark.parametrize("path,tile", [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4)])
 @pytest.mark.parametrize("ert", [0.0, 0.99])
-def test_single_march_views(ert):
+def test_single_march_views(ert, path, tile):
     n = (61, 47, 83)
     v = W.make_cube(W.Recipe(*n, seed=31, n_sources=5))
     s = O.minmax_hist(v)
     R = float(max(abs(s.vmin), abs(s.vmax)))
     tf = W.tf_opaque(n, 0.5) if ert else W.tf_haze(n, 0.5)
     with vr.Volume(dev(v), n) as vol:
+        vol.set_option(vr.VR_OPT_RENDER_PATH, path)
+        vol.set_option(vr.VR_OPT_TILE_SHAPE, tile)
         vol.set_transfer_function(tf, s.vmin, s.vmax)
         for name, cam in _views(n):
             cam = cam.with_(ert_alpha=ert)
             om = O.render(v, cam, O.MIP)
-            check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)
+            sm = check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)
+            assert vol.stats()["path"] == (1 if path == 1 else 4)
             oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
-            st = check_ea(vol.render(cam, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
+            se = check_ea(vol.render(cam, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
+            assert sm["bit_exact"] == 1.0 and se["bit_exact"] == 1.0, (name, sm, se)   # same canonical op sequence
             if ert:
                 assert (oe.K_ert < oe.K).sum() > 20, name          # ERT really fires in this workload
+
+
+@pytest.mark.parametrize("tile", [1, 2, 4])
+def test_tile_wave_many_tiles_ragged(tile):
+    """Several tiles per axis with a ragged last tile (n-1 not a multiple of the tile edge), eye outside on a
+    diagonal and eye inside the volume, ERT on an opaque TF: the wave order must reproduce the k order."""
+    n = (131, 70, 98)
+    v = W.make_cube(W.Recipe(*n, seed=77, n_sources=12))
+    s = O.minmax_hist(v)
+    R = float(max(abs(s.vmin), abs(s.vmax)))
+    tf = W.tf_opaque(n, 0.5)
+    c = np.array(n) / 2
+    cams = [W.perspective_camera(c + np.array([1.1, 0.9, -1.3]) * max(n), c, (0, 1, 0), 35.0, 160, 120, step=0.5),
+            W.perspective_camera((65.5, 33.2, 40.7), (0, 10, 98), (0, 1, 0), 80.0, 128, 96, step=0.5),
+            W.ortho_lookat_camera(c + np.array([0.7, -1.2, 0.4]) * max(n), c, (0, 0, 1), 1.3 * max(n), 120, 90, step=0.75)]
+    with vr.Volume(dev(v), n) as vol:
+        vol.set_option(vr.VR_OPT_RENDER_PATH, vr.VR_PATH_TILE_WAVE)
+        vol.set_option(vr.VR_OPT_TILE_SHAPE, tile)
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for cam in cams:
+            for ert in (0.0, 0.99):
+                cam2 = cam.with_(ert_alpha=ert)
+                oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax)
+                se = check_ea(vol.render(cam2, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
+                assert se["bit_exact"] == 1.0 and vol.stats()["path"] == 4, se
+            om = O.render(v, cam, O.MIP)
+            assert check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)["bit_exact"] == 1.0
+
+
+def test_set_option_rejects_bad_values():
+    v = W.make_cube(W.Recipe(16, 16, 16, seed=1))
+    with vr.Volume(dev(v), (16, 16, 16)) as vol:
+        for opt, val in ((vr.VR_OPT_RENDER_PATH, 3), (vr.VR_OPT_TILE_SHAPE, 9), (77, 0)):
+            with pytest.raises(vr.VrError) as e:
+                vol.set_option(opt, val)
+            assert e.value.status == vr.VR_ERR_INVALID_ARG
 
 
 def test_all_miss_camera_and_eye_inside():
