@@ -265,7 +265,8 @@ def test_host_linear_mirror_and_host_outputs():
         torch.cuda.synchronize()
         oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
         check_ea(out.numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
-        assert vol.stats()["d2h_bytes"] == out.numel() * 4 and vol.stats()["h2d_bytes"] == 0
+        assert vol.stats()["d2h_bytes"] == out.numel() * 4
+        assert vol.stats()["h2d_bytes"] < 4096                           # per-frame tables only; the cube is not re-uploaded
 
 
 def test_pageable_host_memory_is_rejected():
