@@ -104,6 +104,8 @@ struct vr_volume {
     unsigned int tile_serial = 0;
     uint64_t tile_done_sig = 0;               // tile grid the done flags were cleared for
     int opt_path = 0, opt_tile = 0;           // vr_set_option
+    unsigned int *beam_overflow_h = nullptr;  // mapped pinned word the beam kernel sets if a slab box overflowed
+    unsigned int *beam_overflow_d = nullptr;
     Staging staging[kStagingRing];
     int staging_next = 0;
 
@@ -130,6 +132,7 @@ static void free_volume(vr_volume *v)
     if (v->d_tf) cudaFree(v->d_tf);
     if (v->d_sum) cudaFree(v->d_sum);
     if (v->d_sum_out) cudaFree(v->d_sum_out);
+    if (v->beam_overflow_h) cudaFreeHost(v->beam_overflow_h);
     v->arena.release();
     v->host_image.release();
     v->tile_work.release(); v->tile_ctrl.release(); v->tile_done.release();
@@ -456,7 +459,7 @@ static vr_status render_chain(vr_volume *v, const vr_camera *c, const CamK &cam,
 // tile-wave march of a device-resident linear volume (vr_tiles.cu): exact ERT, one pass over the voxels
 static bool tiles_applicable(const vr_volume *v, const vr_camera *c, bool persp, bool ortho)
 {
-    if (v->opt_path == 1) return false;
+    if (v->opt_path != 2) return false;                       // tile-wave only on request (ablation); auto = beam-slab
     if (v->desc.layout != VR_LINEAR || v->out_of_core || !(persp || ortho)) return false;
     (void)c;
     return true;
@@ -541,6 +544,22 @@ static vr_status render_tiles(vr_volume *v, const vr_camera *c, const CamK &cam,
     s->in_flight = true;
     v->stats.path = 4;
     v->stats.bricks_drawn = (uint32_t)n_tiles;
+    return VR_OK;
+}
+
+
+// beam-slab march of a device-resident linear volume (vr_beam.cu): one launch, exact ERT, ray state in registers
+static vr_status render_beam(vr_volume *v, const CamK &cam, int mode, bool ert, const TfK &tf, float *img,
+                             long long pitch_f, cudaStream_t st, bool *applied)
+{
+    VolK V;
+    V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
+    V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz; V.ox = V.oy = V.oz = 0;
+    vr_status rc = launch_beam(mode, ert, cam, V, tf, v->beam_overflow_d, img, pitch_f, st, applied);
+    if (rc != VR_OK || !*applied) return rc;
+    v->stats.kernel_launches += 1;
+    v->stats.path = 5;
+    v->stats.bricks_drawn = (uint32_t)v->n_bricks;
     return VR_OK;
 }
 
@@ -634,6 +653,9 @@ VR_API vr_status vr_create_volume(const vr_volume_desc *d, vr_volume **out)
     VR_FAIL_CUDA(cudaMalloc(&v->d_tf, 257 * sizeof(float4)));
     VR_FAIL_CUDA(cudaMalloc(&v->d_sum, sizeof(SummaryScratch)));
     VR_FAIL_CUDA(cudaMalloc(&v->d_sum_out, VR_SUMMARY_BYTES(4096)));
+    VR_FAIL_CUDA(cudaHostAlloc(&v->beam_overflow_h, sizeof(unsigned int), cudaHostAllocMapped));
+    *v->beam_overflow_h = 0u;
+    VR_FAIL_CUDA(cudaHostGetDevicePointer(&v->beam_overflow_d, v->beam_overflow_h, 0));
 #undef VR_FAIL_CUDA
     *out = v;
     return VR_OK;
@@ -718,7 +740,11 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     if (sort_last) rc = render_sort_last(v, c, cam, mode, tf, img, pitch_f, st);
     else if (v->out_of_core || v->desc.layout == VR_BRICKED_HALO1) rc = render_chain(v, c, cam, mode, ert, tf, img, pitch_f, st);
     else if (tiles_applicable(v, c, persp, ortho)) rc = render_tiles(v, c, cam, mode, ert, persp, tf, img, pitch_f, st);
-    else rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
+    else {
+        bool applied = false;
+        if (v->opt_path != 1 && (persp || ortho)) rc = render_beam(v, cam, mode, ert, tf, img, pitch_f, st, &applied);
+        if (rc == VR_OK && !applied) rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
+    }
     if (rc != VR_OK) return rc;
     VR_CUDA(cudaGetLastError());
     if (im->location == VR_HOST_PINNED) {
@@ -808,7 +834,7 @@ VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
     VR_REQUIRE(v, "vr_set_option: NULL handle");
     switch (option) {
     case VR_OPT_RENDER_PATH:
-        VR_REQUIRE(value >= 0 && value <= 2, "VR_OPT_RENDER_PATH: 0 auto, 1 ray-major, 2 tile-wave (got %lld)", (long long)value);
+        VR_REQUIRE(value >= 0 && value <= 3, "VR_OPT_RENDER_PATH: 0 auto, 1 ray-major, 2 tile-wave, 3 beam-slab (got %lld)", (long long)value);
         v->opt_path = (int)value; return VR_OK;
     case VR_OPT_TILE_SHAPE:
         VR_REQUIRE(value >= 0 && value < VR_TILE_KINDS, "VR_OPT_TILE_SHAPE: 0..%d (got %lld)", VR_TILE_KINDS - 1, (long long)value);
@@ -824,6 +850,7 @@ VR_API vr_status vr_get_stats(vr_volume *v, vr_stats *s)
     VR_REQUIRE(v && s, "vr_get_stats: NULL argument");
     VR_REQUIRE(s->struct_size == sizeof(vr_stats), "vr_stats.struct_size %u != %zu", s->struct_size, sizeof(vr_stats));
     *s = v->stats;
+    s->beam_overflow = v->beam_overflow_h ? *reinterpret_cast<volatile unsigned int *>(v->beam_overflow_h) : 0u;
     return VR_OK;
 }
 

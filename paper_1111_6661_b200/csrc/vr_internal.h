@@ -126,4 +126,12 @@ vr_status launch_tile_march(int kind, int mode, bool ert, const CamK &cam, const
                             const TfK &tf, const TileWork *work, unsigned int *ctrl, unsigned int *done,
                             unsigned int serial, float *image, long long pitch_f, int sm_count, cudaStream_t st);
 
+
+// ---------------------------------------------------------------- beam-slab ray casting (vr_beam.cu)
+// One CTA per 16x16-pixel beam, ray state in registers, the beam's voxel box staged slab by slab in
+// shared memory by TMA (double buffered).  *applied = false: camera / volume outside what the path
+// handles (very wide beams, boxes larger than shared memory) — nothing was enqueued.
+vr_status launch_beam(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, unsigned int *overflow_dev,
+                      float *image, long long pitch_f, cudaStream_t st, bool *applied);
+
 }  // namespace vr

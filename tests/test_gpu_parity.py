@@ -88,7 +88,8 @@ def test_cfg1_full():
     se = check_ea(ea, oe.image)
     assert sm["bit_exact"] == 1.0 and se["bit_exact"] == 1.0        # same canonical op sequence
     assert np.array_equal(ea, ea2)                                   # run-to-run determinism
-    assert st["path"] == 4                                           # auto = tile-wave for a pure ortho camera
+    assert st["path"] == 5 and st["kernel_launches"] == 1           # auto = beam-slab for a pure ortho camera
+    assert st["beam_overflow"] == 0
     assert st_r["path"] == 1 and st_r["kernel_launches"] == 1
     assert check_mip(mip_r, om.image, R)["bit_exact"] == 1.0 and check_ea(ea_r, oe.image)["bit_exact"] == 1.0
 
@@ -101,8 +102,13 @@ def _views(n):
     yield "axis", W.ortho_axis_camera(n, 0, -1, step=1.0)
 
 
-# path 1 = ray-major through global memory; path 2 = tile-wave with each staging-tile shape
-@pytest.mark.parametrize("path,tile", [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4)])
+# path 1 = ray-major through global memory; path 2 = tile-wave with each staging-tile shape; path 3 = beam-slab
+# (nx = 61 is not a multiple of 4, so the beam path runs its plain-load fallback here; the TMA loader is
+# covered by test_beam_slab_tma_views)
+_PATH_ID = {1: 1, 2: 4, 3: 5}
+
+
+@pytest.mark.parametrize("path,tile", [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (3, 0)])
 @pytest.mark.parametrize("ert", [0.0, 0.99])
 def test_single_march_views(ert, path, tile):
     n = (61, 47, 83)
@@ -118,7 +124,7 @@ def test_single_march_views(ert, path, tile):
             cam = cam.with_(ert_alpha=ert)
             om = O.render(v, cam, O.MIP)
             sm = check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)
-            assert vol.stats()["path"] == (1 if path == 1 else 4)
+            assert vol.stats()["path"] == _PATH_ID[path]
             oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
             se = check_ea(vol.render(cam, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
             assert sm["bit_exact"] == 1.0 and se["bit_exact"] == 1.0, (name, sm, se)   # same canonical op sequence
@@ -153,10 +159,63 @@ def test_tile_wave_many_tiles_ragged(tile):
             assert check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)["bit_exact"] == 1.0
 
 
+def _axis_views(n):
+    """Views whose beams travel along +-x, +-y, +-z (all three principal-axis classes, both directions), oblique
+    ones that mix classes across the image, a wide-angle one from inside, and image sizes that are not
+    multiples of the 16x16 beam."""
+    c = np.array(n, dtype=np.float64) / 2
+    m = float(max(n))
+    for k, e in enumerate([(1.6, 0.25, 0.3), (-1.5, -0.2, 0.35), (0.3, 1.7, 0.2), (0.25, -1.6, -0.3),
+                           (0.3, 0.2, 1.8), (-0.2, 0.35, -1.7), (1.2, 1.1, 1.3), (-1.0, 1.2, -1.1)]):
+        up = (0, 0, 1) if abs(e[1]) > 1 else (0, 1, 0)
+        yield f"persp{k}", W.perspective_camera(c + np.array(e) * m, c, up, 42.0, 150, 105, step=0.5)
+    yield "ortho_x", W.ortho_lookat_camera(c + np.array([1.7, 0.4, -0.5]) * m, c, (0, 1, 0), 1.5 * m, 90, 70, step=0.75)
+    yield "ortho_z", W.ortho_lookat_camera(c + np.array([-0.3, 0.5, 1.9]) * m, c, (0, 1, 0), 1.5 * m, 100, 60, step=0.6)
+    yield "inside", W.perspective_camera(c + np.array([0.11, -0.07, 0.2]) * m, c + np.array([0.5, 0.4, -0.3]) * m,
+                                         (0, 1, 0), 75.0, 176, 128, step=0.5)
+    yield "axis_z", W.ortho_axis_camera(n, 2, +1, step=0.5, width=2 * n[0], height=2 * n[1])
+    yield "axis_x", W.ortho_axis_camera(n, 0, -1, step=1.0)
+
+
+@pytest.mark.parametrize("n", [(132, 72, 100), (64, 200, 40)])
+def test_beam_slab_tma_views(n):
+    """Beam-slab path with the TMA loader (nx % 4 == 0): EA with and without ERT and MIP, bit-identical to the
+    oracle's single march (same canonical op sequence), no slab-box overflow."""
+    v = W.make_cube(W.Recipe(*n, seed=91, n_sources=14))
+    s = O.minmax_hist(v)
+    R = float(max(abs(s.vmin), abs(s.vmax)))
+    tf = W.tf_opaque(n, 0.5)
+    with vr.Volume(dev(v), n) as vol:
+        vol.set_option(vr.VR_OPT_RENDER_PATH, vr.VR_PATH_BEAM_SLAB)
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for name, cam in _axis_views(n):
+            for ert in (0.0, 0.99):
+                cam2 = cam.with_(ert_alpha=ert)
+                oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax)
+                se = check_ea(vol.render(cam2, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
+                st = vol.stats()
+                assert st["path"] == 5 and st["beam_overflow"] == 0, (name, st)
+                assert se["bit_exact"] == 1.0, (name, ert, se)
+            om = O.render(v, cam, O.MIP)
+            assert check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)["bit_exact"] == 1.0, name
+
+
+def test_beam_slab_falls_back_for_mixed_camera():
+    """A camera whose origins AND directions vary per pixel is outside the beam path: auto must use ray-major."""
+    n = (32, 32, 32)
+    v = W.make_cube(W.Recipe(*n, seed=3))
+    cam = W.perspective_camera((80.0, 20.0, 16.0), (16, 16, 16), (0, 1, 0), 30.0, 40, 30)
+    cam = cam.with_(ou=np.array([0.01, 0, 0], dtype=np.float32))
+    with vr.Volume(dev(v), n) as vol:
+        g = vol.render(cam, vr.VR_MIP).cpu().numpy()
+        assert vol.stats()["path"] == 1
+    assert np.array_equal(g, O.render(v, cam, O.MIP).image)
+
+
 def test_set_option_rejects_bad_values():
     v = W.make_cube(W.Recipe(16, 16, 16, seed=1))
     with vr.Volume(dev(v), (16, 16, 16)) as vol:
-        for opt, val in ((vr.VR_OPT_RENDER_PATH, 3), (vr.VR_OPT_TILE_SHAPE, 9), (77, 0)):
+        for opt, val in ((vr.VR_OPT_RENDER_PATH, 4), (vr.VR_OPT_TILE_SHAPE, 9), (77, 0)):
             with pytest.raises(vr.VrError) as e:
                 vol.set_option(opt, val)
             assert e.value.status == vr.VR_ERR_INVALID_ARG
