@@ -228,6 +228,8 @@ def run_ours(args):
     frames_step = len(cams) * len(modes)
 
     vol = vr.Volume(dev, cfg.dims, brick=cfg.brick)
+    if args.path:
+        vol.set_option(vr.VR_OPT_RENDER_PATH, args.path)
     sbuf = torch.empty(32 + 8 * 256, dtype=torch.uint8, device="cuda")
     s = vr.Volume.read_summary(vol.minmax_histogram(256, out=sbuf))
     vmin, vmax = float(s["vmin"]), float(s["vmax"])
@@ -362,6 +364,7 @@ def run_ours(args):
             "frames_per_s": world * frames_step / (ms_step * 1e-3),
             "render_ms": {"min": float(np.min(render_ms)), "median": float(np.median(render_ms)),
                           "mean": k_ms, "max": float(np.max(render_ms))},
+            "render_ms_by_view": [round(float(np.mean(render_ms[v::frames_step])), 4) for v in range(frames_step)],
             "render_share_of_step": float(np.sum(render_ms)) / ms_total,
             "effective_hbm_gbs_per_frame": 4.0 * n_vox / (k_ms * 1e-3) / 1e9,
             "samples_per_step": int(samples_step)}
@@ -384,6 +387,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--path", type=int, default=0, help="VR_OPT_RENDER_PATH for ablations (0 = auto, the product default)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -204,7 +204,7 @@ typedef struct {
     uint32_t n_bricks;              /* bricks in the grid */
     uint32_t bricks_drawn;          /* bricks that produced work in the last render */
     uint32_t bricks_culled;         /* bricks outside the view (empty screen rectangle) */
-    uint32_t path;                  /* last render: 0 none, 1 ray-major march, 2 sort-last, 3 brick chain, 4 tile-wave, 5 beam-slab */
+    uint32_t path;                  /* last render: 0 none, 1 ray-major march, 2 sort-last, 3 brick chain, 4 tile-wave, 5 beam-slab (TMA boxes), 6 sheared-plane beams */
     uint32_t kernel_launches;       /* library kernels launched by the last call */
     uint64_t fragments;             /* (brick,pixel) partial fragments written (sort-last) */
     uint64_t h2d_bytes;             /* host-to-device bytes enqueued by the last call */
@@ -212,7 +212,9 @@ typedef struct {
     uint64_t total_kernel_launches; /* since vr_create_volume */
     uint64_t resident_bytes;        /* device bytes owned by the handle */
     uint32_t beam_overflow;         /* != 0: a beam-slab box exceeded its planned capacity (internal error; never expected) */
-    uint32_t reserved;
+    uint32_t beams_direct_total;    /* beams of the sheared-plane path marched from global memory because their planes
+                                       did not fit a shared-memory slot, since vr_create_volume (valid once the renders
+                                       have completed) */
 } vr_stats;
 
 VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
@@ -222,11 +224,12 @@ VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
  * tolerances (all paths evaluate the same canonical arithmetic, C.1-C.7); used by the parity
  * tests to force each path and by bench.py for ablations.
  *   VR_OPT_RENDER_PATH  how a device-resident VR_LINEAR volume is marched when VR_SORT_LAST is
- *                       not requested: 0 = auto (beam-slab when the camera is purely perspective
- *                       or purely orthographic and its beams fit shared memory, else ray-major),
- *                       1 = ray-major (one thread per ray through global memory), 2 = tile-wave
- *                       (shared-memory tiles in dataflow order; kept for ablation), 3 = beam-slab
- *                       (falls back to ray-major like auto).
+ *                       not requested: 0 = auto (sheared-plane beams when the camera is purely
+ *                       perspective or purely orthographic and its beams fit shared memory, else
+ *                       ray-major), 1 = ray-major (one thread per ray through global memory),
+ *                       2 = tile-wave (shared-memory tiles in dataflow order; kept for ablation),
+ *                       3 = beam-slab with TMA slab boxes (kept for ablation), 4 = sheared-plane
+ *                       beams (3 and 4 fall back to ray-major like auto).
  *   VR_OPT_TILE_SHAPE   staging tile of the tile-wave path: 0 = auto, 1 = 32x32x32,
  *                       2 = 32x32x16, 3 = 32x16x16, 4 = 16x16x16 ownership cells.
  * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).

@@ -19,7 +19,7 @@ VR_DEVICE, VR_HOST_PINNED = 0, 1
 VR_EA, VR_MIP = 0, 1
 VR_SORT_LAST = 1
 VR_OPT_RENDER_PATH, VR_OPT_TILE_SHAPE = 1, 2
-VR_PATH_AUTO, VR_PATH_RAY_MAJOR, VR_PATH_TILE_WAVE, VR_PATH_BEAM_SLAB = 0, 1, 2, 3
+VR_PATH_AUTO, VR_PATH_RAY_MAJOR, VR_PATH_TILE_WAVE, VR_PATH_BEAM_SLAB, VR_PATH_SHEAR = 0, 1, 2, 3, 4
 
 _STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_UNSUPPORTED", 3: "VR_ERR_OUT_OF_MEMORY",
            4: "VR_ERR_CUDA", 5: "VR_ERR_NOT_READY"}
@@ -54,7 +54,7 @@ class vr_stats(C.Structure):
                 ("bricks_culled", C.c_uint32), ("path", C.c_uint32), ("kernel_launches", C.c_uint32),
                 ("fragments", C.c_uint64), ("h2d_bytes", C.c_uint64), ("d2h_bytes", C.c_uint64),
                 ("total_kernel_launches", C.c_uint64), ("resident_bytes", C.c_uint64),
-                ("beam_overflow", C.c_uint32), ("reserved", C.c_uint32)]
+                ("beam_overflow", C.c_uint32), ("beams_direct_total", C.c_uint32)]
 
 
 EXPORTS = ("vr_create_volume", "vr_destroy_volume", "vr_set_transfer_function", "vr_render",

@@ -104,7 +104,7 @@ struct vr_volume {
     unsigned int tile_serial = 0;
     uint64_t tile_done_sig = 0;               // tile grid the done flags were cleared for
     int opt_path = 0, opt_tile = 0;           // vr_set_option
-    unsigned int *beam_overflow_h = nullptr;  // mapped pinned word the beam kernel sets if a slab box overflowed
+    unsigned int *beam_overflow_h = nullptr;  // mapped pinned words: [0] set if a staged box / plane overflowed, [1] beams marched from global memory
     unsigned int *beam_overflow_d = nullptr;
     Staging staging[kStagingRing];
     int staging_next = 0;
@@ -459,7 +459,7 @@ static vr_status render_chain(vr_volume *v, const vr_camera *c, const CamK &cam,
 // tile-wave march of a device-resident linear volume (vr_tiles.cu): exact ERT, one pass over the voxels
 static bool tiles_applicable(const vr_volume *v, const vr_camera *c, bool persp, bool ortho)
 {
-    if (v->opt_path != 2) return false;                       // tile-wave only on request (ablation); auto = beam-slab
+    if (v->opt_path != 2) return false;                       // tile-wave only on request (ablation)
     if (v->desc.layout != VR_LINEAR || v->out_of_core || !(persp || ortho)) return false;
     (void)c;
     return true;
@@ -563,6 +563,21 @@ static vr_status render_beam(vr_volume *v, const CamK &cam, int mode, bool ert, 
     return VR_OK;
 }
 
+// sheared-plane beam march of a device-resident linear volume (vr_shear.cu): one launch, exact ERT
+static vr_status render_shear(vr_volume *v, const CamK &cam, int mode, bool ert, const TfK &tf, float *img,
+                              long long pitch_f, cudaStream_t st, bool *applied)
+{
+    VolK V;
+    V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
+    V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz; V.ox = V.oy = V.oz = 0;
+    vr_status rc = launch_shear(mode, ert, cam, V, tf, v->beam_overflow_d, img, pitch_f, st, applied);
+    if (rc != VR_OK || !*applied) return rc;
+    v->stats.kernel_launches += 1;
+    v->stats.path = 6;
+    v->stats.bricks_drawn = (uint32_t)v->n_bricks;
+    return VR_OK;
+}
+
 }  // namespace vr
 
 // ====================================================================== C ABI
@@ -653,8 +668,8 @@ VR_API vr_status vr_create_volume(const vr_volume_desc *d, vr_volume **out)
     VR_FAIL_CUDA(cudaMalloc(&v->d_tf, 257 * sizeof(float4)));
     VR_FAIL_CUDA(cudaMalloc(&v->d_sum, sizeof(SummaryScratch)));
     VR_FAIL_CUDA(cudaMalloc(&v->d_sum_out, VR_SUMMARY_BYTES(4096)));
-    VR_FAIL_CUDA(cudaHostAlloc(&v->beam_overflow_h, sizeof(unsigned int), cudaHostAllocMapped));
-    *v->beam_overflow_h = 0u;
+    VR_FAIL_CUDA(cudaHostAlloc(&v->beam_overflow_h, 2 * sizeof(unsigned int), cudaHostAllocMapped));
+    v->beam_overflow_h[0] = v->beam_overflow_h[1] = 0u;
     VR_FAIL_CUDA(cudaHostGetDevicePointer(&v->beam_overflow_d, v->beam_overflow_h, 0));
 #undef VR_FAIL_CUDA
     *out = v;
@@ -742,7 +757,10 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     else if (tiles_applicable(v, c, persp, ortho)) rc = render_tiles(v, c, cam, mode, ert, persp, tf, img, pitch_f, st);
     else {
         bool applied = false;
-        if (v->opt_path != 1 && (persp || ortho)) rc = render_beam(v, cam, mode, ert, tf, img, pitch_f, st, &applied);
+        if ((v->opt_path == 0 || v->opt_path == 4) && (persp || ortho))
+            rc = render_shear(v, cam, mode, ert, tf, img, pitch_f, st, &applied);
+        if (rc == VR_OK && !applied && v->opt_path == 3 && (persp || ortho))
+            rc = render_beam(v, cam, mode, ert, tf, img, pitch_f, st, &applied);
         if (rc == VR_OK && !applied) rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
     }
     if (rc != VR_OK) return rc;
@@ -834,7 +852,7 @@ VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
     VR_REQUIRE(v, "vr_set_option: NULL handle");
     switch (option) {
     case VR_OPT_RENDER_PATH:
-        VR_REQUIRE(value >= 0 && value <= 3, "VR_OPT_RENDER_PATH: 0 auto, 1 ray-major, 2 tile-wave, 3 beam-slab (got %lld)", (long long)value);
+        VR_REQUIRE(value >= 0 && value <= 4, "VR_OPT_RENDER_PATH: 0 auto, 1 ray-major, 2 tile-wave, 3 beam-slab (TMA), 4 sheared planes (got %lld)", (long long)value);
         v->opt_path = (int)value; return VR_OK;
     case VR_OPT_TILE_SHAPE:
         VR_REQUIRE(value >= 0 && value < VR_TILE_KINDS, "VR_OPT_TILE_SHAPE: 0..%d (got %lld)", VR_TILE_KINDS - 1, (long long)value);
@@ -850,7 +868,8 @@ VR_API vr_status vr_get_stats(vr_volume *v, vr_stats *s)
     VR_REQUIRE(v && s, "vr_get_stats: NULL argument");
     VR_REQUIRE(s->struct_size == sizeof(vr_stats), "vr_stats.struct_size %u != %zu", s->struct_size, sizeof(vr_stats));
     *s = v->stats;
-    s->beam_overflow = v->beam_overflow_h ? *reinterpret_cast<volatile unsigned int *>(v->beam_overflow_h) : 0u;
+    s->beam_overflow = v->beam_overflow_h ? reinterpret_cast<volatile unsigned int *>(v->beam_overflow_h)[0] : 0u;
+    s->beams_direct_total = v->beam_overflow_h ? reinterpret_cast<volatile unsigned int *>(v->beam_overflow_h)[1] : 0u;
     return VR_OK;
 }
 

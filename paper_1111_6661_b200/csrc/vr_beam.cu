@@ -35,6 +35,7 @@
 #include <cstring>
 #include <vector>
 
+#include "vr_beamgeom.cuh"
 #include "vr_internal.h"
 
 namespace vr {
@@ -42,64 +43,12 @@ namespace vr {
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kBW = 16, kBH = 16;                    // beam = 16 x 16 pixels, 8 warps of 8 x 4
-constexpr int kStrip = 16;                           // beams per strip row (scheduling order)
-constexpr float kMargin = 0.05f;                     // voxels; >> float32 error of any position (< 2e-3 at 2^14)
 constexpr unsigned kTfBytes = 257 * 16;              // transfer function
 constexpr unsigned kCtlOff = kTfBytes;               // 2 mbarriers (16 B) + control words
 constexpr unsigned kBufOff = 4352;                   // first stage buffer (multiple of 128)
 constexpr unsigned kSmemMax = 232448;                // 227 KB per CTA (B200)
 
-// ------------------------------------------------------------------ geometry shared by the host plan and the kernel
-struct BeamLine { float Au, Ru, Av, Rv; };           // transverse position on the plane p_a = c:  p_u = Au + c Ru
-
-__host__ __device__ inline void beam_axes(int a, int &u, int &v) { u = a == 0 ? 1 : 0; v = a == 2 ? 1 : 2; }
-
-__host__ __device__ inline void cam_ray_at(const CamK &c, float px, float py, float o[3], float g[3])
-{
-    for (int a = 0; a < 3; ++a) {
-        o[a] = fmaf(py, c.ov[a], fmaf(px, c.ou[a], c.o0[a]));
-        g[a] = fmaf(py, c.dv[a], fmaf(px, c.du[a], c.d0[a]));
-    }
-}
-
-// z before y before x on ties: the longer the contiguous rows of a slab box, the better for TMA
-__host__ __device__ inline int principal_axis(const float g[3])
-{
-    const float ax = fabsf(g[0]), ay = fabsf(g[1]), az = fabsf(g[2]);
-    return (az >= ax && az >= ay) ? 2 : (ay >= ax ? 1 : 0);
-}
-
-// the line of the ray through pixel-space point (px,py), parameterised by the principal coordinate.
-// false: the ray does not travel along `sgn` of axis a, or is more oblique than |d_a| = 0.3.
-__host__ __device__ inline bool beam_line(const CamK &c, float px, float py, int a, int sgn, BeamLine &L)
-{
-    float o[3], g[3];
-    cam_ray_at(c, px, py, o, g);
-    int u, v;
-    beam_axes(a, u, v);
-    const float ga = g[a], len2 = g[0] * g[0] + g[1] * g[1] + g[2] * g[2];
-    if (!(ga * (float)sgn > 0.0f) || !(ga * ga >= 0.09f * len2)) return false;
-    L.Ru = g[u] / ga; L.Rv = g[v] / ga;
-    L.Au = o[u] - o[a] * L.Ru; L.Av = o[v] - o[a] * L.Rv;
-    return true;
-}
-
-// the two planes that bound the sample positions a slab of base indices [lo, hi] can own (C.7:
-// ownership cell [lo + 1/2, hi + 3/2), outer cells reach the volume faces)
-__host__ __device__ inline void slab_planes(int lo, int hi, int na, float &cA, float &cB)
-{
-    cA = lo <= 0 ? 0.0f : (float)lo + 0.5f;
-    cB = hi >= na - 2 ? (float)na : (float)hi + 1.5f;
-}
-
-__host__ __device__ inline int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
-
-__host__ __device__ inline int floor_clamped(float q)
-{
-    q = fminf(fmaxf(q, -1.0e6f), 1.0e6f);
-    return (int)floorf(q);
-}
+// beam geometry (BeamLine, beam_line, slab_planes, ...): vr_beamgeom.cuh
 
 struct BeamPlanK {
     int tiles_x, tiles_y;

@@ -88,7 +88,7 @@ def test_cfg1_full():
     se = check_ea(ea, oe.image)
     assert sm["bit_exact"] == 1.0 and se["bit_exact"] == 1.0        # same canonical op sequence
     assert np.array_equal(ea, ea2)                                   # run-to-run determinism
-    assert st["path"] == 5 and st["kernel_launches"] == 1           # auto = beam-slab for a pure ortho camera
+    assert st["path"] == 6 and st["kernel_launches"] == 1           # auto = sheared-plane beams for a pure ortho camera
     assert st["beam_overflow"] == 0
     assert st_r["path"] == 1 and st_r["kernel_launches"] == 1
     assert check_mip(mip_r, om.image, R)["bit_exact"] == 1.0 and check_ea(ea_r, oe.image)["bit_exact"] == 1.0
@@ -104,11 +104,11 @@ def _views(n):
 
 # path 1 = ray-major through global memory; path 2 = tile-wave with each staging-tile shape; path 3 = beam-slab
 # (nx = 61 is not a multiple of 4, so the beam path runs its plain-load fallback here; the TMA loader is
-# covered by test_beam_slab_tma_views)
-_PATH_ID = {1: 1, 2: 4, 3: 5}
+# covered by test_beam_views); path 4 = sheared-plane beams (the default)
+_PATH_ID = {0: 6, 1: 1, 2: 4, 3: 5, 4: 6}
 
 
-@pytest.mark.parametrize("path,tile", [(1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (3, 0)])
+@pytest.mark.parametrize("path,tile", [(0, 0), (1, 0), (2, 1), (2, 2), (2, 3), (2, 4), (3, 0), (4, 0)])
 @pytest.mark.parametrize("ert", [0.0, 0.99])
 def test_single_march_views(ert, path, tile):
     n = (61, 47, 83)
@@ -177,16 +177,18 @@ def _axis_views(n):
     yield "axis_x", W.ortho_axis_camera(n, 0, -1, step=1.0)
 
 
-@pytest.mark.parametrize("n", [(132, 72, 100), (64, 200, 40)])
-def test_beam_slab_tma_views(n):
-    """Beam-slab path with the TMA loader (nx % 4 == 0): EA with and without ERT and MIP, bit-identical to the
+@pytest.mark.parametrize("path", [3, 4])
+@pytest.mark.parametrize("n", [(132, 72, 100), (64, 200, 40), (61, 47, 83)])
+def test_beam_views(n, path):
+    """Both beam paths (3: TMA slab boxes when nx % 4 == 0, else its plain loader; 4: sheared planes by
+    cp.async) over views travelling along +-x, +-y, +-z: EA with and without ERT and MIP, bit-identical to the
     oracle's single march (same canonical op sequence), no slab-box overflow."""
     v = W.make_cube(W.Recipe(*n, seed=91, n_sources=14))
     s = O.minmax_hist(v)
     R = float(max(abs(s.vmin), abs(s.vmax)))
     tf = W.tf_opaque(n, 0.5)
     with vr.Volume(dev(v), n) as vol:
-        vol.set_option(vr.VR_OPT_RENDER_PATH, vr.VR_PATH_BEAM_SLAB)
+        vol.set_option(vr.VR_OPT_RENDER_PATH, path)
         vol.set_transfer_function(tf, s.vmin, s.vmax)
         for name, cam in _axis_views(n):
             for ert in (0.0, 0.99):
@@ -194,7 +196,7 @@ def test_beam_slab_tma_views(n):
                 oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax)
                 se = check_ea(vol.render(cam2, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
                 st = vol.stats()
-                assert st["path"] == 5 and st["beam_overflow"] == 0, (name, st)
+                assert st["path"] == _PATH_ID[path] and st["beam_overflow"] == 0, (name, st)
                 assert se["bit_exact"] == 1.0, (name, ert, se)
             om = O.render(v, cam, O.MIP)
             assert check_mip(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image, R)["bit_exact"] == 1.0, name
@@ -215,7 +217,7 @@ def test_beam_slab_falls_back_for_mixed_camera():
 def test_set_option_rejects_bad_values():
     v = W.make_cube(W.Recipe(16, 16, 16, seed=1))
     with vr.Volume(dev(v), (16, 16, 16)) as vol:
-        for opt, val in ((vr.VR_OPT_RENDER_PATH, 4), (vr.VR_OPT_TILE_SHAPE, 9), (77, 0)):
+        for opt, val in ((vr.VR_OPT_RENDER_PATH, 5), (vr.VR_OPT_TILE_SHAPE, 9), (77, 0)):
             with pytest.raises(vr.VrError) as e:
                 vol.set_option(opt, val)
             assert e.value.status == vr.VR_ERR_INVALID_ARG
