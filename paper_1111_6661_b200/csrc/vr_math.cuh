@@ -15,6 +15,26 @@ __device__ __forceinline__ float lerp_ee(float a, float b, float f)
     return __fmaf_rn(f, b, __fmaf_rn(-f, a, a));
 }
 
+// Two independent correctly rounded float32 fused multiply-adds in one instruction (sm_100 FFMA2):
+// (a.x*b.x + c.x, a.y*b.y + c.y).  Same results as two __fmaf_rn; halves the issue slots of the lerps.
+__device__ __forceinline__ float2 fma2_rn(float2 a, float2 b, float2 c)
+{
+    unsigned long long ua, ub, uc, ud;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(uc) : "f"(c.x), "f"(c.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(ub), "l"(uc));
+    float2 d;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(ud));
+    return d;
+}
+
+// exact-ends lerp of two pairs with one fraction: (L(a.x,b.x,f), L(a.y,b.y,f))
+__device__ __forceinline__ float2 lerp_ee2(float2 a, float2 b, float f)
+{
+    return fma2_rn(make_float2(f, f), b, fma2_rn(make_float2(-f, -f), a, a));
+}
+
 struct CamK {                       // kernel-side copy of vr_camera (C.1)
     float o0[3], ou[3], ov[3], d0[3], du[3], dv[3];
     float step;
@@ -91,6 +111,16 @@ __device__ __forceinline__ float trilerp(float v000, float v100, float v010, flo
     const float c0 = lerp_ee(c00, c10, fy);
     const float c1 = lerp_ee(c01, c11, fy);
     return lerp_ee(c0, c1, fz);
+}
+
+// C.3 with the x and y lerps paired over z (same operations and operands as trilerp, 8 instructions)
+__device__ __forceinline__ float trilerp_packed(float v000, float v100, float v010, float v110, float v001, float v101,
+                                                float v011, float v111, float fx, float fy, float fz)
+{
+    const float2 c0x = lerp_ee2(make_float2(v000, v001), make_float2(v100, v101), fx);      // (c00, c01)
+    const float2 c1x = lerp_ee2(make_float2(v010, v011), make_float2(v110, v111), fx);      // (c10, c11)
+    const float2 cy = lerp_ee2(c0x, c1x, fy);                                               // (c0, c1)
+    return lerp_ee(cy.x, cy.y, fz);
 }
 
 // C.4: post-interpolative classification from a 257-entry shared-memory table (entry 256 is a

@@ -47,8 +47,9 @@ constexpr unsigned kSmemMax = 232448;                // 227 KB per CTA (B200)
 constexpr unsigned kSmemSM = 233472;                 // 228 KB per SM, 1 KB reserved per resident CTA
 
 // shared-memory map (bytes)
-constexpr unsigned kTfOff = 0;                       // float2 tf[4][256]: (T[i][c], T[i+1][c]) pairs
-constexpr unsigned kTfBytes = 4 * 256 * 8;
+constexpr unsigned kTfOff = 0;                       // float2 rg[257] at + 0, float2 ba[257] at + kTfBA (entry i = T[i])
+constexpr unsigned kTfBA = 2064;
+constexpr unsigned kTfBytes = 2 * kTfBA;
 constexpr unsigned kCtlOff = kTfOff + kTfBytes;      // int ctl[8]
 constexpr unsigned kLineOff = kCtlOff + 32;          // BeamLine line[4]
 constexpr unsigned kStepOff = kLineOff + 64;         // StepRec step[3]
@@ -62,9 +63,10 @@ struct StepRec {               // one step: march base planes [wlo, wlo + wn) af
 struct LoadRec {               // one plane to stage
     int q, u0, v0, w, h;       // plane index along a; rectangle origin and size (u, v)
     unsigned int sdst;         // shared-memory byte address of voxel (u0, v0) of the plane
-    int pad0, pad1;
+    const float *g0;           // global address of voxel (u0, v0) of the plane
 };
 
+static_assert(sizeof(LoadRec) == 32 && sizeof(StepRec) == 32, "plan records are addressed with fixed byte offsets");
 enum { kCtlMin = 0, kCtlMax = 1, kCtlDirect = 2 };
 
 struct ShearPlanK {
@@ -108,6 +110,13 @@ __device__ __forceinline__ unsigned int lds_u32(unsigned int a)
     return v;
 }
 template <int OFF>
+__device__ __forceinline__ unsigned long long lds_u64(unsigned int a)
+{
+    unsigned long long v;
+    asm volatile("ld.shared.u64 %0, [%1+%2];" : "=l"(v) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF>
 __device__ __forceinline__ float2 lds_f32x2(unsigned int a)
 {
     float2 v;
@@ -138,8 +147,8 @@ __device__ __forceinline__ float sample_global(const VolK &V, const Ray &r, floa
                    __ldg(pz + V.sy), __ldg(pz + V.sy + 1), fx, fy, fz);
 }
 
-// C.4 from the pair table at shared address tfa: pair (T[i][c], T[i+1][c]) at tfa + 2048 c + 8 i;
-// same arithmetic as classify() of vr_math.cuh
+// C.4 from the two half tables at shared address tfa ((r,g) of entry i at tfa + 8 i, (b,a) at + kTfBA); same
+// arithmetic as classify() of vr_math.cuh with the four channel lerps paired
 __device__ __forceinline__ float4 classify_pairs(unsigned int tfa, float scale, float bias, float s)
 {
     const float u = __saturatef(__fmaf_rn(s, scale, bias));
@@ -147,8 +156,19 @@ __device__ __forceinline__ float4 classify_pairs(unsigned int tfa, float scale, 
     const int i = min(__float2int_rz(x), 254);
     const float f = __fsub_rn(x, (float)i);
     const unsigned int e = tfa + 8u * (unsigned int)i;
-    const float2 r = lds_f32x2<0>(e), g = lds_f32x2<2048>(e), b = lds_f32x2<4096>(e), a = lds_f32x2<6144>(e);
-    return make_float4(lerp_ee(r.x, r.y, f), lerp_ee(g.x, g.y, f), lerp_ee(b.x, b.y, f), lerp_ee(a.x, a.y, f));
+    const float2 rg = lerp_ee2(lds_f32x2<0>(e), lds_f32x2<8>(e), f);
+    const float2 ba = lerp_ee2(lds_f32x2<kTfBA>(e), lds_f32x2<kTfBA + 8>(e), f);
+    return make_float4(rg.x, rg.y, ba.x, ba.y);
+}
+
+// C.5 with the r and g accumulations paired
+__device__ __forceinline__ void composite_packed(float4 rgba, float &Cr, float &Cg, float &Cb, float &T)
+{
+    const float w = __fmul_rn(T, rgba.w);
+    const float2 c = fma2_rn(make_float2(w, w), make_float2(rgba.x, rgba.y), make_float2(Cr, Cg));
+    Cr = c.x; Cg = c.y;
+    Cb = __fmaf_rn(w, rgba.z, Cb);
+    T = __fsub_rn(T, w);
 }
 
 // ------------------------------------------------------------------ per-beam state shared by the helpers
@@ -157,6 +177,8 @@ struct BeamCtx {
     int sgn, na, nu, nv;
     int G, NS, PU, PV, PP;
     int iw_min, iw_max;
+    const float *vbase;        // volume base and the element strides of the plane index, u and v
+    long long sq, su, sv;
     unsigned int *overflow;
     // shared memory: generic views (warp 0 writes the plan through these) and shared-space addresses (reads)
     BeamLine *lines;
@@ -193,6 +215,7 @@ __device__ __forceinline__ void plan_step(const BeamCtx &B, int rec, bool first,
         B.tab[q & 63] = tv; B.tab[(q & 63) + 64] = tv;
         LoadRec &R = B.loads[rec * 20 + lane];
         R.q = q; R.u0 = u0; R.v0 = v0; R.w = w; R.h = h; R.sdst = sdst;
+        R.g0 = B.vbase + ((long long)q * B.sq + (long long)u0 * B.su + (long long)v0 * B.sv);
     }
     const int wmax = __reduce_max_sync(0xffffffffu, w), hmax = __reduce_max_sync(0xffffffffu, h);
     next_ord += nload;
@@ -218,14 +241,14 @@ __device__ __forceinline__ void load_planes(const BeamCtx &B, const VolK &V, int
     if (nload == 0) return;
     const unsigned int PU4 = 4u * (unsigned int)B.PU;
     if (A != 0) {
-        const long long sa = A == 2 ? V.sz : V.sy, sv = A == 2 ? V.sy : V.sz;
+        const long long sv = A == 2 ? V.sy : V.sz;
+        const long long goff = (long long)warp * sv + lane;                  // this thread's first element of a plane
+        const unsigned int soff = PU4 * (unsigned int)warp + 4u * (unsigned int)lane;
         for (int k = 0; k < nload; ++k) {
             const unsigned int la = B.load_a + 32u * (unsigned int)(rec * 20 + k);
-            const int q = (int)lds_u32<0>(la), u0 = (int)lds_u32<4>(la), v0 = (int)lds_u32<8>(la);
             const int w = (int)lds_u32<12>(la), h = (int)lds_u32<16>(la);
-            const unsigned int sdst = lds_u32<20>(la);
-            const float *g = V.base + ((long long)q * sa + (long long)(v0 + warp) * sv + (u0 + lane));
-            unsigned int s = sdst + PU4 * (unsigned int)warp + 4u * (unsigned int)lane;
+            const float *g = reinterpret_cast<const float *>(lds_u64<24>(la)) + goff;
+            unsigned int s = lds_u32<20>(la) + soff;
             for (int x0 = 0; x0 < w; x0 += 64) {                       // one pass unless a plane is wider than 64
                 const bool p0 = lane + x0 < w, p1 = lane + x0 + 32 < w;
                 const float *gr = g + x0;
@@ -249,12 +272,10 @@ __device__ __forceinline__ void load_planes(const BeamCtx &B, const VolK &V, int
         const int pl = lane & ((1 << sh) - 1), sub = lane >> sh, per = 32 >> sh;
         const bool act = pl < nload;
         const unsigned int la = B.load_a + 32u * (unsigned int)(rec * 20 + (act ? pl : 0));
-        const int q = (int)lds_u32<0>(la), u0 = (int)lds_u32<4>(la), v0 = (int)lds_u32<8>(la);
         const int w = act ? (int)lds_u32<12>(la) : 0, h = act ? (int)lds_u32<16>(la) : 0;
-        const unsigned int sdst = lds_u32<20>(la);
         const int wmax = (int)lds_u32<12>(sa_rec), hmax = (int)lds_u32<16>(sa_rec);
-        const float *g = V.base + ((long long)(v0 + warp) * V.sz + (long long)(u0 + sub) * V.sy + q);
-        unsigned int s = sdst + PU4 * (unsigned int)warp + 4u * (unsigned int)sub;
+        const float *g = reinterpret_cast<const float *>(lds_u64<24>(la)) + ((long long)warp * V.sz + (long long)sub * V.sy);
+        unsigned int s = lds_u32<20>(la) + PU4 * (unsigned int)warp + 4u * (unsigned int)sub;
         const long long gstep = (long long)per * V.sy;
         const unsigned int sstep = 4u * (unsigned int)per;
         for (int r = warp; r < hmax; r += kWarps) {
@@ -298,12 +319,12 @@ __device__ __forceinline__ void march_step(const BeamCtx &B, const VolK &V, cons
         const float q00 = lds_f32<0>(a0), q10 = lds_f32<4>(a0), q01 = lds_f32<0>(a0v), q11 = lds_f32<4>(a0v);
         const float p00 = lds_f32<0>(a1), p10 = lds_f32<4>(a1), p01 = lds_f32<0>(a1v), p11 = lds_f32<4>(a1v);
         float sv;
-        if (A == 2)      sv = trilerp(q00, q10, q01, q11, p00, p10, p01, p11, fx, fy, fz);   // a = z, u = x, v = y
-        else if (A == 1) sv = trilerp(q00, q10, p00, p10, q01, q11, p01, p11, fx, fy, fz);   // a = y, u = x, v = z
-        else             sv = trilerp(q00, p00, q10, p10, q01, p01, q11, p11, fx, fy, fz);   // a = x, u = y, v = z
+        if (A == 2)      sv = trilerp_packed(q00, q10, q01, q11, p00, p10, p01, p11, fx, fy, fz);   // a = z, u = x, v = y
+        else if (A == 1) sv = trilerp_packed(q00, q10, p00, p10, q01, q11, p01, p11, fx, fy, fz);   // a = y, u = x, v = z
+        else             sv = trilerp_packed(q00, p00, q10, p10, q01, p01, q11, p11, fx, fy, fz);   // a = x, u = y, v = z
         if (MODE == VR_MIP) acc.m = fmaxf(acc.m, sv);
         else {
-            composite(classify_pairs(B.tf_a, scale, bias, sv), acc.cr, acc.cg, acc.cb, acc.T);
+            composite_packed(classify_pairs(B.tf_a, scale, bias, sv), acc.cr, acc.cg, acc.cb, acc.T);
             if (ERT && acc.T <= cam.t_min) { alive = false; break; }         // stop AFTER compositing this sample (C.5)
         }
         kf = __fadd_rn(kf, 1.0f);                                            // exact: k < 2^24
@@ -358,10 +379,10 @@ k_shear(CamK cam, VolK V, TfK tf, ShearPlanK P, float *__restrict__ image, long 
 
     if (threadIdx.x == 0) { ctl[kCtlMin] = INT_MAX; ctl[kCtlMax] = INT_MIN; ctl[kCtlDirect] = 0; }
     if (MODE == VR_EA)
-        for (int e = threadIdx.x; e < 1024; e += kThreads) {
-            const int c = e >> 8, k = e & 255;
-            const float *t0 = reinterpret_cast<const float *>(tf.table + k) + c;
-            tfp[e] = make_float2(__ldg(t0), __ldg(t0 + 4));                      // entry 256 is the pad copy of 255
+        for (int e = threadIdx.x; e < 257; e += kThreads) {                      // entry 256 is the pad copy of 255
+            const float4 t = __ldg(tf.table + e);
+            tfp[e] = make_float2(t.x, t.y);
+            *reinterpret_cast<float2 *>(smem + kTfOff + kTfBA + 8 * e) = make_float2(t.z, t.w);
         }
 
     // principal axis and direction of travel of this beam (uniform: from the beam centre)
@@ -386,6 +407,10 @@ k_shear(CamK cam, VolK V, TfK tf, ShearPlanK P, float *__restrict__ image, long 
     B.PV = a == 0 ? P.PV[0] : a == 1 ? P.PV[1] : P.PV[2];
     B.PP = a == 0 ? P.PP[0] : a == 1 ? P.PP[1] : P.PP[2];
     B.overflow = P.overflow;
+    B.vbase = V.base;
+    B.sq = a == 0 ? 1 : a == 1 ? V.sy : V.sz;
+    B.su = a == 0 ? V.sy : 1;
+    B.sv = a == 2 ? V.sy : V.sz;
     B.lines = reinterpret_cast<BeamLine *>(smem + kLineOff);
     B.steps = reinterpret_cast<StepRec *>(smem + kStepOff);
     B.tab = reinterpret_cast<unsigned int *>(smem + kTabOff);

@@ -357,3 +357,76 @@ def test_two_handles_two_streams_and_pitch():
         assert np.array_equal(ia.cpu().numpy(), O.render(a, cam, O.MIP).image)
         assert np.array_equal(ib.cpu().numpy(), O.render(b, cam, O.MIP).image)
         assert (big[:, 70:] == 0).all()
+
+
+# ------------------------------------------------------------------ full-size configs, bench launch configuration
+def _host_cube(cfg):
+    """The config's cube in host memory, filled in z-slabs by the shared generator (as bench.py does)."""
+    nx, ny, nz = cfg.dims
+    out = np.empty((nz, ny, nx), dtype=np.float32)
+    gen = W.CubeGenerator(cfg.recipe)
+    slab = max(1, (1 << 28) // (nx * ny))
+    for z0 in range(0, nz, slab):
+        z1 = min(nz, z0 + slab)
+        gen.fill(out[z0:z1], z0, z1)
+    return out
+
+
+def _lattice(cfg, stride=8):
+    m = np.zeros((cfg.height, cfg.width), dtype=np.uint8)
+    m[stride // 2::stride, stride // 2::stride] = 1
+    return m
+
+
+def _full_size_case(number, views, summary_exact=True):
+    """vr_minmax_histogram on the whole cube (bit-exact) and vr_render of `views` at the config's own image
+    size, step, ERT and flags — the launches bench.py times — compared with the oracle on a lattice of every
+    8th pixel in x and y (C.11), which the oracle computes ray by ray."""
+    cfg = W.get_config(number)
+    v = _host_cube(cfg)
+    d = torch.from_numpy(v).cuda()
+    tf = W.tf_haze(cfg.dims, cfg.step)
+    mask = _lattice(cfg)
+    sel = mask.astype(bool)
+    with vr.Volume(d, cfg.dims, brick=cfg.brick) as vol:
+        g = gpu_summary(vol)
+        if summary_exact:
+            assert_summary_equal(g, O.minmax_hist(v))
+        vmin, vmax = float(g["vmin"]), float(g["vmax"])
+        R = max(abs(vmin), abs(vmax))
+        vol.set_transfer_function(tf, vmin, vmax)
+        for view in views:
+            cam = cfg.camera(view)
+            for mode in cfg.modes:
+                if mode == "mip":
+                    o = O.render(v, cam, O.MIP, brick=cfg.brick if cfg.sort_last else 0, mask=mask)
+                    gi = vol.render(cam, vr.VR_MIP).cpu().numpy()
+                    s = check_mip(gi[sel], o.image[sel], R)
+                else:
+                    o = O.render(v, cam, O.EA, tf, vmin, vmax, brick=cfg.brick if cfg.sort_last else 0, mask=mask)
+                    gi = vol.render(cam, vr.VR_EA).cpu().numpy()
+                    s = check_ea(gi[sel], o.image[sel], o.fragile[sel], (o.K > 0)[sel])
+                st = vol.stats()
+                assert st["beam_overflow"] == 0
+                assert s["bit_exact"] == 1.0, (number, view, mode, s)      # same canonical op sequence
+                assert o.n_nominal > 1000
+    del d
+    torch.cuda.empty_cache()
+
+
+def test_cfg2_full_size_sampled():
+    """cfg2 (512x512x1024, 1024^2, step 0.5, EA + ERT 0.99): a z-class, a mixed and an x-class orbit view."""
+    _full_size_case(2, views=(0, 2, 3))
+
+
+def test_cfg3_full_size_sampled():
+    """cfg3 (1024x1024x2048, 8 GiB; summary pass; 1920x1080 MIP + EA, 128^3 bricks, sort-last compositing)."""
+    if torch.cuda.get_device_properties(0).total_memory < 24 << 30:
+        pytest.skip("needs 24 GB of device memory")
+    _full_size_case(3, views=(1,))
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("VR_TEST_BIG"), reason="64 GiB cube: set VR_TEST_BIG=1 (takes minutes)")
+def test_cfg4_full_size_sampled():
+    """cfg4 (2048x2048x4096, 64 GiB resident; 3840x2160, step 1, EA + ERT): one orbit view on the pixel lattice."""
+    _full_size_case(4, views=(5,), summary_exact=True)

@@ -103,3 +103,14 @@ def test_configs_shapes():
     assert abs(c2.meta["R"] - 1639) < 1.0
     tf = W.tf_haze((512, 512, 1024), 0.5)
     assert tf.shape == (256, 4) and tf.min() >= 0 and tf.max() <= 1 and tf[0, 3] == 0
+
+
+def test_fill_bricked_halo_layerwise_equals_retile():
+    """The layer-by-layer generator of the brick-major layout (used for cubes that do not fit host memory twice)
+    writes the same bytes as retiling the whole linear cube."""
+    r = W.Recipe(21, 18, 23, seed=99, n_sources=2)
+    for B in (4, 7, 16, 32):
+        ref = W.retile_halo(W.make_cube(r), B)
+        out = np.empty(W.bricked_halo_elems((r.nx, r.ny, r.nz), B), dtype=np.float32)
+        W.fill_bricked_halo_ptr(r, B, out.ctypes.data)
+        assert np.array_equal(out.reshape(ref.shape).view(np.uint32), ref.view(np.uint32))

@@ -46,6 +46,8 @@ def _load():
         lib.vrgen_checksum.argtypes = [C.c_void_p, C.c_uint64]
         lib.vrgen_retile_halo.restype = C.c_int
         lib.vrgen_retile_halo.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p]
+        lib.vrgen_retile_halo_layer.restype = C.c_int
+        lib.vrgen_retile_halo_layer.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p]
         lib.vrgen_det_log.restype = C.c_double
         lib.vrgen_det_log.argtypes = [C.c_double]
         lib.vrgen_det_exp_neg.restype = C.c_double
@@ -139,6 +141,30 @@ def retile_halo(lin: np.ndarray, brick: int) -> np.ndarray:
     if _load().vrgen_retile_halo(lin.ctypes.data, nx, ny, nz, brick, out.ctypes.data) != 0:
         raise ValueError("vrgen_retile_halo failed")
     return out
+
+
+def bricked_halo_elems(dims, brick: int) -> int:
+    """Number of float32 elements of the brick-major (B+1)^3 layout of a cube of ``dims`` = (nx, ny, nz)."""
+    nx, ny, nz = dims
+    return -(-nx // brick) * -(-ny // brick) * -(-nz // brick) * (brick + 1) ** 3
+
+
+def fill_bricked_halo_ptr(recipe: Recipe, brick: int, ptr: int) -> None:
+    """Generate the recipe's cube straight into brick-major-with-halo layout at raw host address ``ptr``
+    (e.g. a pinned torch tensor), one brick layer at a time: the linear cube is never held as a whole."""
+    lib = _load()
+    gen = CubeGenerator(recipe)
+    nx, ny, nz = recipe.nx, recipe.ny, recipe.nz
+    E3 = (brick + 1) ** 3
+    per_layer = -(-nx // brick) * -(-ny // brick)
+    for bz in range(-(-nz // brick)):
+        z0, z1 = bz * brick, min(bz * brick + brick + 1, nz)
+        slab = np.empty((z1 - z0, ny, nx), dtype=np.float32)
+        gen.fill(slab, z0, z1)
+        dst = ptr + 4 * bz * per_layer * E3
+        if lib.vrgen_retile_halo_layer(slab.ctypes.data, nx, ny, z1 - z0, brick, C.c_void_p(dst)) != 0:
+            raise ValueError("vrgen_retile_halo_layer failed")
+        del slab
 
 
 def det_log(x: float) -> float:

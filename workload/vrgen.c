@@ -329,6 +329,36 @@ VRGEN_EXPORT int vrgen_retile_halo(const float *lin, uint32_t nx, uint32_t ny, u
     return 0;
 }
 
+/* One brick LAYER (all bricks with the same bz) from a slab that holds the slices [bz*B, bz*B + nzs), nzs <= B + 1:
+ * the slab is the layer's own z-range plus, unless it is the last layer, its one-slice halo.  Lets a cube
+ * larger than spare host memory be generated straight into the brick-major layout, layer by layer. */
+VRGEN_EXPORT int vrgen_retile_halo_layer(const float *slab, uint32_t nx, uint32_t ny, uint32_t nzs,
+                                         uint32_t B, float *out)
+{
+    if (!slab || !out || !B || !nzs || nzs > B + 1) return -1;
+    uint32_t nbx = (nx + B - 1) / B, nby = (ny + B - 1) / B;
+    uint32_t E = B + 1;
+    int64_t nb = (int64_t)nbx * nby;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t b = 0; b < nb; ++b) {
+        uint32_t bx = (uint32_t)(b % nbx), by = (uint32_t)(b / nbx);
+        float *o = out + (size_t)b * E * E * E;
+        for (uint32_t z = 0; z < E; ++z) {
+            uint32_t gz = z; if (gz > nzs - 1) gz = nzs - 1;
+            for (uint32_t y = 0; y < E; ++y) {
+                uint32_t gy = by * B + y; if (gy > ny - 1) gy = ny - 1;
+                const float *src = slab + (size_t)nx * (gy + (size_t)ny * gz);
+                float *dst = o + (size_t)E * (y + (size_t)E * z);
+                for (uint32_t x = 0; x < E; ++x) {
+                    uint32_t gx = bx * B + x; if (gx > nx - 1) gx = nx - 1;
+                    dst[x] = src[gx];
+                }
+            }
+        }
+    }
+    return 0;
+}
+
 /* test hooks: the deterministic elementary functions */
 VRGEN_EXPORT double vrgen_det_log(double x) { return det_log(x); }
 VRGEN_EXPORT double vrgen_det_exp_neg(double a) { return det_exp_neg(a); }
