@@ -215,6 +215,10 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     cfg = W.get_config(args.config)
+    if cfg.out_of_core:
+        if dist is not None:
+            dist.destroy_process_group()
+        return run_ours_ooc(args, cfg)
     nx, ny, nz = cfg.dims
     n_vox = nx * ny * nz
     host = make_host_cube(cfg, pinned=True)
@@ -377,6 +381,188 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------------- out-of-core arm (cfg5)
+def host_mem_available() -> int:
+    try:
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemAvailable:"):
+                    return int(line.split()[1]) * 1024
+    except Exception:
+        pass
+    return 64 << 30
+
+
+def ooc_config(cfg, nz_arg: int):
+    """cfg5 needs 4096x4096x3072 in pinned host memory as 256^3(+1) bricks = 209 GB.  When the box cannot pin
+    that (SURVEY H7 fallback b) the spectral axis is cut to whole brick layers that fit a third of the available
+    host memory; everything else (brick size, image, views, step, streams) is cfg5's."""
+    from dataclasses import replace
+    import workload as W
+    nx, ny, nz = cfg.dims
+    B = cfg.brick
+    layer_bytes = 4 * W.bricked_halo_elems((nx, ny, B), B)
+    if nz_arg <= 0:
+        fit = int(host_mem_available() / 3 // layer_bytes)
+        nz_arg = min(nz, max(1, fit) * B)
+    if nz_arg >= nz:
+        return cfg, "full size"
+    nz_arg = max(B, nz_arg // B * B)
+    rec = replace(cfg.recipe, nz=nz_arg, n_sources=max(1, cfg.recipe.n_sources * nz_arg // nz))
+    return replace(cfg, recipe=rec, name=f"{cfg.name}@nz{nz_arg}"), f"spectral axis cut from {nz} to {nz_arg} channels: the box cannot pin the full 209 GB"
+
+
+def measure_h2d_peak(stream) -> float:
+    """Host-link peak as SURVEY 8(d) defines it: pinned 1 GiB cudaMemcpyAsync, best of 10, GB/s."""
+    import torch
+    h = torch.empty(1 << 30, dtype=torch.uint8).pin_memory()
+    d = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    best = 0.0
+    for _ in range(10):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream); d.copy_(h, non_blocking=True); b.record(stream); torch.cuda.synchronize()
+        best = max(best, (1 << 30) / (a.elapsed_time(b) * 1e-3) / 1e9)
+    del h, d
+    return best
+
+
+def run_ours_ooc(args, cfg):
+    """cfg5: the cube lives in pinned host memory as brick-major 256^3(+1 halo) bricks; a fixed part of the brick
+    pool stays resident, the rest is streamed per frame in view order on 4 copy streams (A5).  `value` times steps
+    on one handle (resident part already loaded); `e2e` creates the handle inside every step."""
+    import torch
+    import paper_1111_6661_b200 as vr
+    import workload as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg, size_note = ooc_config(cfg, args.ooc_nz)
+    nx, ny, nz = cfg.dims
+    B = cfg.brick
+    n_el = W.bricked_halo_elems(cfg.dims, B)
+    host = torch.empty(n_el, dtype=torch.float32, pin_memory=True)
+    W.fill_bricked_halo_ptr(cfg.recipe, B, host.data_ptr())
+    cube_bytes = 4 * n_el
+    resident = int(args.ooc_resident_frac * cube_bytes)
+    stream = torch.cuda.current_stream()
+    link_peak = measure_h2d_peak(stream)
+    cams = [cfg.camera(v) for v in range(cfg.n_views)]
+    cam_structs = [vr.make_camera(c) for c in cams]
+    samples_step = sum(W.nominal_samples(c, cfg.dims) for c in cams)
+    tf = W.tf_haze(cfg.dims, cfg.step)
+    img = torch.empty((cfg.height, cfg.width, 4), dtype=torch.float32, device="cuda")
+    h_img = torch.empty((cfg.height, cfg.width, 4), dtype=torch.float32).pin_memory()
+    h_sum = torch.empty(32 + 8 * 256, dtype=torch.uint8).pin_memory()
+    frame_ms, frame_h2d, sum_ms, sum_h2d = [], [], [], []
+    last_range = [0.0, 1.0]
+
+    def step(vol, out_img, record):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 + len(cam_structs))]
+        ev[0].record(stream)
+        vol.minmax_histogram(256, out=h_sum)
+        h2d_s = vol.stats()["h2d_bytes"]
+        ev[1].record(stream)
+        stream.synchronize()
+        hs = vr.Volume.read_summary(h_sum)
+        last_range[0], last_range[1] = float(hs["vmin"]), float(hs["vmax"])
+        vol.set_transfer_function(tf, last_range[0], last_range[1])
+        h2d_f = []
+        for k, c in enumerate(cam_structs):
+            vol.render(c, vr.VR_EA, out=out_img)
+            h2d_f.append(vol.stats()["h2d_bytes"])
+            ev[2 + k].record(stream)
+        stream.synchronize()
+        if record:
+            sum_ms.append(ev[0].elapsed_time(ev[1])); sum_h2d.append(h2d_s)
+            for k in range(len(cam_structs)):
+                frame_ms.append(ev[1 + k].elapsed_time(ev[2 + k])); frame_h2d.append(h2d_f[k])
+        return h2d_s + sum(h2d_f)
+
+    vol = vr.Volume(host, cfg.dims, brick=B, layout=vr.VR_BRICKED_HALO1, resident_bytes=resident,
+                    n_copy_streams=cfg.n_copy_streams)
+    for _ in range(args.warmup):
+        step(vol, img, False)
+    torch.cuda.synchronize()
+    clocks = ClockSampler(physical_gpu_index(local)); clocks.start()
+    launches0 = vol.stats()["total_kernel_launches"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    h2d_step = 0
+    for _ in range(args.steps):
+        h2d_step = step(vol, img, True)
+    e1.record(stream); torch.cuda.synchronize()
+    clk = clocks.finish()
+    ms_step = e0.elapsed_time(e1) / args.steps
+    launches = vol.stats()["total_kernel_launches"] - launches0
+    vol.close()
+
+    e2e_steps = max(1, min(args.steps, 2))
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    e2e_h2d = 0
+    for _ in range(e2e_steps):
+        with vr.Volume(host, cfg.dims, brick=B, layout=vr.VR_BRICKED_HALO1, resident_bytes=resident,
+                       n_copy_streams=cfg.n_copy_streams) as hv:
+            e2e_h2d = step(hv, h_img, False)
+    b.record(stream); torch.cuda.synchronize()
+    e2e_ms = a.elapsed_time(b) / e2e_steps
+    if dist is not None:
+        t = torch.tensor([ms_step, e2e_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step, e2e_ms = float(t[0]), float(t[1])
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    k_ms = float(np.mean(frame_ms))
+    gbs = float(np.sum(frame_h2d)) / (float(np.sum(frame_ms)) * 1e-3) / 1e9
+    sum_gbs = float(np.sum(sum_h2d)) / (float(np.sum(sum_ms)) * 1e-3) / 1e9
+    block = config_block(cfg, f"out of core: {size_note}; cube {cube_bytes / 1e9:.1f} GB pinned host, brick-major "
+                              f"{B}^3(+1 halo), resident cap {resident / 1e9:.1f} GB, {cfg.n_copy_streams} copy streams")
+    block["cube_bytes"] = cube_bytes
+    line = {"metric": "voxel_samples_per_s", "value": world * samples_step / (ms_step * 1e-3), "unit": "samples/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": block, "clocks": clk,
+            "e2e": {"value": world * samples_step / (e2e_ms * 1e-3), "unit": "samples/s",
+                    "h2d_bytes_per_step": int(e2e_h2d), "d2h_bytes_per_step": int(len(cams) * h_img.numel() * 4 + 32 + 8 * 256),
+                    "ms_per_step": e2e_ms, "steps": e2e_steps},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "host_link", "achieved": gbs, "peak": link_peak, "unit": "GB/s", "frac": gbs / link_peak,
+                         "traffic": None, "kernel": "vr_render, out-of-core brick chain (cudaMemcpyAsync on the copy streams "
+                         "+ k_chain_brick per brick)", "kernel_ms": k_ms, "launches_timed": len(frame_ms),
+                         "peak_source": "pinned 1 GiB cudaMemcpyAsync, best of 10, measured in this run",
+                         "algorithmic_bytes_per_launch": float(np.mean(frame_h2d))},
+            "summary_pass": {"h2d_gbs": sum_gbs, "frac_of_link": sum_gbs / link_peak, "ms": float(np.mean(sum_ms)),
+                             "h2d_bytes": int(np.mean(sum_h2d))},
+            "frames_per_s": world * len(cams) / (ms_step * 1e-3),
+            "render_ms": {"min": float(np.min(frame_ms)), "median": float(np.median(frame_ms)), "mean": k_ms,
+                          "max": float(np.max(frame_ms))},
+            "h2d_bytes_per_step": int(h2d_step), "samples_per_step": int(samples_step), "cpu_baseline": None}
+    if world == 1 and not args.no_cpu:
+        import oracle as O
+        cam = cfg.camera(0)
+        mask = np.zeros((cam.height, cam.width), dtype=np.uint8)
+        mask[4::8, 4::8] = 1
+        hn = host.numpy().reshape(-1, B + 1, B + 1, B + 1)
+        t0 = time.perf_counter()
+        r = O.render(hn, cam, O.EA, tf, last_range[0], last_range[1], mask=mask, layout=O.BRICKED_HALO1,
+                     layout_brick=B, dims=cfg.dims)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": r.n_nominal / dt, "unit": "samples/s", "cores": O.num_threads(), "kind": "oracle",
+                                "sample": f"{cfg.name} view 0, every 8th pixel in x and y ({r.n_nominal} nominal samples, "
+                                          f"{dt:.2f} s), f32-canonical oracle on the brick-major cube, OpenMP"}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -387,6 +573,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--ooc-nz", type=int, default=0, help="cfg5: spectral channels to use (0 = as many brick layers as fit host memory)")
+    ap.add_argument("--ooc-resident-frac", type=float, default=0.25, help="cfg5: device brick pool as a fraction of the cube")
     ap.add_argument("--path", type=int, default=0, help="VR_OPT_RENDER_PATH for ablations (0 = auto, the product default)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -232,9 +232,12 @@ VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
  *                       beams (3 and 4 fall back to ray-major like auto).
  *   VR_OPT_TILE_SHAPE   staging tile of the tile-wave path: 0 = auto, 1 = 32x32x32,
  *                       2 = 32x32x16, 3 = 32x16x16, 4 = 16x16x16 ownership cells.
+ *   VR_OPT_SPARSE_DIRECT  experimental, default 0.  1: in the sheared-plane path, beams whose planes contain
+ *                       x and whose rays would stage more than ~6 voxels per sample (sparse sampling: several
+ *                       voxels per pixel) skip the staging and read through L1.  Same arithmetic, same results.
  * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).
  * ------------------------------------------------------------------------------------------ */
-enum { VR_OPT_RENDER_PATH = 1, VR_OPT_TILE_SHAPE = 2 };
+enum { VR_OPT_RENDER_PATH = 1, VR_OPT_TILE_SHAPE = 2, VR_OPT_SPARSE_DIRECT = 3 };
 VR_API vr_status vr_set_option(vr_volume *vol, uint32_t option, int64_t value);
 
 /* Thread-local message of the last failing call on this thread ("" if none). */

@@ -18,7 +18,7 @@ VR_LINEAR, VR_BRICKED_HALO1 = 0, 1
 VR_DEVICE, VR_HOST_PINNED = 0, 1
 VR_EA, VR_MIP = 0, 1
 VR_SORT_LAST = 1
-VR_OPT_RENDER_PATH, VR_OPT_TILE_SHAPE = 1, 2
+VR_OPT_RENDER_PATH, VR_OPT_TILE_SHAPE, VR_OPT_SPARSE_DIRECT = 1, 2, 3
 VR_PATH_AUTO, VR_PATH_RAY_MAJOR, VR_PATH_TILE_WAVE, VR_PATH_BEAM_SLAB, VR_PATH_SHEAR = 0, 1, 2, 3, 4
 
 _STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_UNSUPPORTED", 3: "VR_ERR_OUT_OF_MEMORY",

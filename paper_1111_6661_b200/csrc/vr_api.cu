@@ -103,7 +103,7 @@ struct vr_volume {
     DevBuf<unsigned int> tile_ctrl, tile_done;
     unsigned int tile_serial = 0;
     uint64_t tile_done_sig = 0;               // tile grid the done flags were cleared for
-    int opt_path = 0, opt_tile = 0;           // vr_set_option
+    int opt_path = 0, opt_tile = 0, opt_sparse = 0;   // vr_set_option
     unsigned int *beam_overflow_h = nullptr;  // mapped pinned words: [0] set if a staged box / plane overflowed, [1] beams marched from global memory
     unsigned int *beam_overflow_d = nullptr;
     Staging staging[kStagingRing];
@@ -570,7 +570,7 @@ static vr_status render_shear(vr_volume *v, const CamK &cam, int mode, bool ert,
     VolK V;
     V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
     V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz; V.ox = V.oy = V.oz = 0;
-    vr_status rc = launch_shear(mode, ert, cam, V, tf, v->beam_overflow_d, img, pitch_f, st, applied);
+    vr_status rc = launch_shear(mode, ert, v->opt_sparse != 0, cam, V, tf, v->beam_overflow_d, img, pitch_f, st, applied);
     if (rc != VR_OK || !*applied) return rc;
     v->stats.kernel_launches += 1;
     v->stats.path = 6;
@@ -857,6 +857,9 @@ VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
     case VR_OPT_TILE_SHAPE:
         VR_REQUIRE(value >= 0 && value < VR_TILE_KINDS, "VR_OPT_TILE_SHAPE: 0..%d (got %lld)", VR_TILE_KINDS - 1, (long long)value);
         v->opt_tile = (int)value; return VR_OK;
+    case VR_OPT_SPARSE_DIRECT:
+        VR_REQUIRE(value == 0 || value == 1, "VR_OPT_SPARSE_DIRECT: 0 or 1 (got %lld)", (long long)value);
+        v->opt_sparse = (int)value; return VR_OK;
     default:
         set_error("unknown option %u", option); return VR_ERR_INVALID_ARG;
     }

@@ -74,6 +74,8 @@ struct ShearPlanK {
     int G[3];                  // planes per step per principal-axis class
     int NS[3];                 // ring slots per class (>= 2 G + 1)
     int PU[3], PV[3], PP[3];   // row pitch, rows, plane pitch (words) per class
+    int sparse[3];             // 1: beams of this class sample so sparsely that staging whole planes costs more than
+                               //    it saves; they march through global memory (host plan, see launch_shear)
     unsigned int *overflow;    // mapped host words: [0] set to 1 if a plane ever exceeded its slot (never expected),
                                // [1] counts the beams marched from global memory
 };
@@ -452,7 +454,9 @@ k_shear(CamK cam, VolK V, TfK tf, ShearPlanK P, float *__restrict__ image, long 
 
     // ---- warp 0: the four corner lines of the beam, the fit test, the plans of the first two steps
     int next_ord = 0, wstart = 0;
-    if (warp == 0) {
+    const bool sparse_class = (a == 0 ? P.sparse[0] : a == 1 ? P.sparse[1] : P.sparse[2]) != 0;
+    if (warp == 0 && sparse_class) { if (lane == 0) ctl[kCtlDirect] = 1; }
+    if (warp == 0 && !sparse_class) {
         BeamLine Lm = { 0.0f, 0.0f, 0.0f, 0.0f };
         const float cx = (float)((lane & 1) ? min(x0 + kBW, cam.width) : x0);
         const float cy = (float)((lane & 2) ? min(y0 + kBH, cam.height) : y0);
@@ -558,8 +562,8 @@ void plan_caps(const CamK &cam, const int n[3], int tiles_x, int tiles_y, int ca
 
 // Enqueues one frame.  *applied = false (and VR_OK) if nothing was enqueued because not even three plane slots
 // fit shared memory (the caller then uses another path).
-vr_status launch_shear(int mode, bool ert, const CamK &cam, const VolK &V, const TfK &tf, unsigned int *overflow_dev,
-                       float *image, long long pitch_f, cudaStream_t st, bool *applied)
+vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, const VolK &V, const TfK &tf,
+                       unsigned int *overflow_dev, float *image, long long pitch_f, cudaStream_t st, bool *applied)
 {
     *applied = false;
     const int n[3] = { V.nx, V.ny, V.nz };
@@ -575,6 +579,22 @@ vr_status launch_shear(int mode, bool ert, const CamK &cam, const VolK &V, const
     // Per class: the ring of 2 G + 1 plane slots with the largest G that leaves room for three CTAs per SM
     // (if G >= 3), else for two (G >= 2), else for one; else shrink the slots (beams that then do not fit
     // march from global memory).  Class 0 loads with G + 1 lanes per cell, so there G + 1 is a power of two.
+    // VR_OPT_SPARSE_DIRECT (experimental, off by default; not yet measured end to end).  Sparse sampling (cfg4:
+    // 1.7-3.3 voxels per pixel, step 1): neighbouring rays share no voxel, so staging a whole plane rectangle
+    // moves cap_w * cap_h / 256 words per ray and plane for the 8 a ray reads.  Measured on cfg4 with the
+    // separate kernels (BENCH_NOTES.md): views whose planes contain x march faster straight through L1 (lanes
+    // along x share sectors: 19 ms against 38 ms for a z-class view); x-principal views do not (169 ms against
+    // 88 ms: through L1 every lane touches its own line).  With the option set, beams of classes 1 and 2 that
+    // would stage more than ~6 words per sample march through global memory.
+    for (int a = 1; a < 3 && sparse_direct; ++a) {
+        if (cap[a][0] == 0) continue;
+        float oc[3], gc[3];
+        cam_ray_at(cam, 0.5f * (float)W, 0.5f * (float)H, oc, gc);
+        const float len = std::sqrt(gc[0] * gc[0] + gc[1] * gc[1] + gc[2] * gc[2]);
+        const float per_plane = std::max(1.0f / (cam.step * std::max(std::fabs(gc[a]) / len, 0.3f)), 1.0f);   // samples per plane
+        const float words = (float)cap[a][0] * (float)cap[a][1] / (float)(kBW * kBH);
+        if (words / per_plane > 6.0f) { P.sparse[a] = 1; cap[a][0] = cap[a][1] = 0; }
+    }
     bool fits = false;
     unsigned int ring_words = 0;
     for (int shrink = 0; shrink < 24 && !fits; ++shrink) {

@@ -430,3 +430,24 @@ def test_cfg3_full_size_sampled():
 def test_cfg4_full_size_sampled():
     """cfg4 (2048x2048x4096, 64 GiB resident; 3840x2160, step 1, EA + ERT): one orbit view on the pixel lattice."""
     _full_size_case(4, views=(5,), summary_exact=True)
+
+
+def test_sparse_direct_option_same_results():
+    """VR_OPT_SPARSE_DIRECT (experimental): sparse views (several voxels per pixel) of classes 1 and 2 read through
+    L1 instead of staging planes — same canonical arithmetic, so bit-identical images."""
+    n = (96, 80, 112)
+    v = W.make_cube(W.Recipe(*n, seed=57, n_sources=6))
+    s = O.minmax_hist(v)
+    tf = W.tf_opaque(n, 1.0)
+    c = np.array(n, dtype=np.float64) / 2
+    cams = [W.perspective_camera(c + np.array(e) * 140.0, c, up, 50.0, 40, 28, step=1.0, ert_alpha=0.99)
+            for e, up in (((0.2, 0.3, 1.7), (0, 1, 0)), ((0.3, 1.6, 0.2), (0, 0, 1)), ((1.7, 0.2, 0.3), (0, 1, 0)))]
+    with vr.Volume(dev(v), n) as vol:
+        vol.set_option(vr.VR_OPT_SPARSE_DIRECT, 1)
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for cam in cams:
+            oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
+            se = check_ea(vol.render(cam, vr.VR_EA).cpu().numpy(), oe.image, oe.fragile, oe.K > 0, max_fragile_frac=0.05)
+            assert se["bit_exact"] == 1.0 and vol.stats()["path"] == 6 and vol.stats()["beam_overflow"] == 0
+            om = O.render(v, cam, O.MIP)
+            assert np.array_equal(vol.render(cam, vr.VR_MIP).cpu().numpy(), om.image)
