@@ -107,6 +107,22 @@ def physical_gpu_index(local: int) -> int:
     return local
 
 
+def max_over_ranks(values, dist, device):
+    """Element-wise MAX of a list of floats over all ranks (identity without a process group): the timing rule
+    of the contract — every multi-rank number is the slowest rank's."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def aggregate_value(units_per_rank: float, world: int, ms_step: float) -> float:
+    """Whole-job throughput of N independent replicas (weak scaling): units all ranks processed / slowest time."""
+    return world * units_per_rank / (ms_step * 1e-3)
+
+
 # ---------------------------------------------------------------------------------- workload
 def make_host_cube(cfg, pinned=True):
     """The config's seeded cube in (pinned) host memory, filled in z-slabs by the shared generator."""
@@ -281,12 +297,9 @@ def run_ours(args):
     launches = vol.stats()["total_kernel_launches"] - launches0
     render_ms = [a.elapsed_time(b) for a, b in ev_pairs]
     path = vol.stats()["path"]
-    if dist is not None:
-        t = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks([ms_total], dist, "cuda")[0]
     ms_step = ms_total / args.steps
-    value = world * samples_step / (ms_step * 1e-3)
+    value = aggregate_value(samples_step, world, ms_step)
 
     # ---- end to end through the C ABI with host buffers (every step uploads the cube)
     h_sum = torch.empty(32 + 8 * 256, dtype=torch.uint8).pin_memory()
@@ -323,11 +336,8 @@ def run_ours(args):
         b.record(stream)
         barrier()
         e2e_ms = a.elapsed_time(b)
-    if dist is not None:
-        t = torch.tensor([e2e_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e_value = world * samples_step / (e2e_ms / e2e_steps * 1e-3)
+    e2e_ms = max_over_ranks([e2e_ms], dist, "cuda")[0]
+    e2e_value = aggregate_value(samples_step, world, e2e_ms / e2e_steps)
 
     if rank != 0:
         if dist is not None:
@@ -512,10 +522,7 @@ def run_ours_ooc(args, cfg):
             e2e_h2d = step(hv, h_img, False)
     b.record(stream); torch.cuda.synchronize()
     e2e_ms = a.elapsed_time(b) / e2e_steps
-    if dist is not None:
-        t = torch.tensor([ms_step, e2e_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step, e2e_ms = float(t[0]), float(t[1])
+    ms_step, e2e_ms = max_over_ranks([ms_step, e2e_ms], dist, "cuda")
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
