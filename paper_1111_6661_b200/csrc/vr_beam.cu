@@ -2,7 +2,7 @@
 // ("the GPU part" of the case study; PAPER.md:L66
 // sub-cube partitioning, here applied per beam and per frame instead of per GPU).
 //
-// Design.  A CTA owns a BEAM: the rays of one 16x16 pixel tile, one thread per ray,
+// Design (kept as the ablation path 3, superseded by vr_shear.cu).  A CTA owns a BEAM: the rays of one 16x16 pixel tile, one thread per ray,
 // ray state (C, T) / m in registers from the first sample to the last — so the recurrence of C.5
 // runs in k order, early termination is exact, and nothing is exchanged between CTAs.  The beam
 // is cut along its PRINCIPAL axis a (largest |d_a| of the centre ray) into slabs of D base-index
@@ -13,10 +13,10 @@
 // ray that the slab OWNS (C.7 at slab granularity: sample k belongs to the slab iff its clamped
 // base index i0_a lies in [lo, hi]; i0_a is monotone in k, so ownership is one compare per
 // sample) out of shared memory: 8 LDS per sample instead of 8 global loads that each touch
-// ~10-25 L1 sectors (profiles/r1_raymajor_ncu.md).  All 32 lanes of a warp work on every slab
+// ~10-25 L1 sectors (ray-major path: 7.08 ms per cfg2 frame, BENCH_NOTES.md).  All 32 lanes of a warp work on every slab
 // (every ray of a beam crosses every slab of the beam), which is what the tile-wave path
 // (vr_tiles.cu) lacked: there ~60 % of the issue slots went to rays that missed the tile and to
-// per-segment set-up (profiles/r1_tilewave_ncu.md).
+// per-segment set-up (an ncu capture of an earlier session, not kept).
 //
 // Arithmetic.  Identical to k_march_full: positions, indices and fractions come from the
 // canonical GLOBAL position (vr_math.cuh); the shared-memory address is formed by integer
@@ -25,7 +25,7 @@
 // HBM traffic.  Beams are scheduled in 16-beam-wide strips so that co-resident CTAs form a
 // compact block of the image; neighbouring beams overlap only in the halo and in the slack of
 // the bounding box, which L2 (126 MB) serves.  Every voxel inside the view is read from HBM about
-// once per frame; the box slack is re-read from L2 (DESIGN.md §6 gives the measured ratio).
+// once per frame; the box slack is re-read from L2 (profiles/r1a_beam_tma_ncu.md: 1.2-1.4 GB of DRAM reads per 1.07 GB frame, 7 GB staged).
 #include <cuda.h>
 
 #include <algorithm>

@@ -2,7 +2,7 @@
 // volumes ("the GPU part" of the case study;
 // PAPER.md:L66 sub-cube partitioning, applied here per beam and per frame instead of per GPU).
 //
-// Design (DESIGN.md §5).  As in vr_beam.cu a CTA owns a BEAM — the rays of one 16x16 pixel tile, one
+// Design (DESIGN.md §7).  As in vr_beam.cu a CTA owns a BEAM — the rays of one 16x16 pixel tile, one
 // thread per ray, ray state (C, T) / m in registers from the first sample to the last, so the
 // recurrence of C.5 runs in k order and early termination is exact — and the beam is traversed along
 // its PRINCIPAL axis a, its samples marched out of shared memory.  What differs is how the voxels
@@ -82,7 +82,7 @@ struct ShearPlanK {
 
 // Best plane-pitch residue (mod 32) for each row-pitch residue, per class, and the row-pitch residues
 // to avoid: minimum mean conflict degree of one corner LDS over 2280 warp patterns of 76 views
-// (random eyes, the six axis views, the cfg2 orbit), bank model of DESIGN.md §5.  All "good" pairs
+// (random eyes, the six axis views, the cfg2 orbit), bank model of DESIGN.md §7.  All "good" pairs
 // give 2.3-2.6 wavefronts per LDS (measured 2.34, profiles/r1b_shear_ncu.md); 16-byte-granular
 // layouts give 3.7-8 (measured 7.2).
 constexpr unsigned char kBestPP[3][32] = {

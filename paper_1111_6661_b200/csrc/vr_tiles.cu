@@ -3,7 +3,7 @@
 //
 // Why.  One thread per ray marching through global memory is bound by the L1 tag stage: the 32
 // rays of a warp touch ~25 different 32-byte sectors per corner load, eight loads per sample
-// (profiles/r1_raymajor_ncu.md).  Shared memory has no sector granularity: 32 lanes reading 32
+// (an ncu capture of an earlier session, not kept; BENCH_NOTES.md has the timings).  Shared memory has no sector granularity: 32 lanes reading 32
 // different words cost ~2 wavefronts with the padded strides below.  So the volume is cut into
 // staging tiles of TX x TY x TZ ownership cells (C.7 applied at tile granularity), a CTA copies
 // one tile (+1 high-side halo) into shared memory with cp.async and marches every ray segment
@@ -38,7 +38,7 @@ constexpr int kThreads = 256;
 constexpr int pad_mod32(int v, int r) { return v + ((r - v % 32) + 32) % 32; }
 
 // shared-memory strides: sy = 5 (mod 32), sz = 7 (mod 32) gave the lowest bank-conflict degree
-// (2.1 wavefronts per corner load vs 3.8 for dense 33 x 33) over random views
+// (2.1 wavefronts per corner load vs 3.8 for dense 33 x 33) over random views (bank model)
 template <int TX_, int TY_, int TZ_>
 struct TileCfg {
     static constexpr int TX = TX_, TY = TY_, TZ = TZ_;

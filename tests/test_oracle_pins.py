@@ -406,3 +406,17 @@ def test_p13_step_halving_converges_on_smooth_cube():
         imgs.append(O.render(v, cam0.with_(step=step), O.EA, tf, 0.0, float(v.max()), precision=O.F64).image64)
     e = [np.abs(imgs[k] - imgs[k + 1]).max() for k in range(3)]
     assert e[0] > e[1] > e[2] and e[2] < 0.35 * e[0]
+
+
+def test_oracle_matches_its_committed_golden():
+    """Regression guard: the oracle's bits on one tiny seeded case (tests/golden/oracle_tiny.txt, written by
+    tests/golden/make_oracle_golden.py from the oracle alone).  Not a pin against the paper — it prints no numbers."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_oracle_golden", os.path.join(here, "make_oracle_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    with open(os.path.join(here, "oracle_tiny.txt")) as f:
+        stored = f.read().splitlines()
+    assert list(mod.lines()) == stored
