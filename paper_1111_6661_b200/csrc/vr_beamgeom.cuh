@@ -66,7 +66,8 @@ __host__ __device__ inline int floor_clamped(float q)
 
 // Voxels of DATA plane P (index along the principal axis) that samples of the beam bounded by the four
 // corner lines L[0..3] can read.  Plane P is read by samples whose base index is P - 1 or P, i.e. whose
-// principal coordinate lies in [P - 1/2, P + 3/2] (clipped to the volume); between two planes the beam is
+// principal coordinate lies in [P - 1/2, P + 3/2] (to the volume face for the outer base indices, which
+// also own the outer half voxel); between two planes the beam is
 // the convex hull of its corner lines, so the extremes are taken at the corners on the two end planes.
 // A sample at transverse coordinate p reads base index floor(p - 1/2) (clamped to [0, n-2]) and its +1
 // neighbour.  raw: widths before the clamp to the volume (a convex function of P: checking both ends of a
@@ -74,7 +75,8 @@ __host__ __device__ inline int floor_clamped(float q)
 __host__ __device__ inline void plane_rect(const BeamLine L[4], int P, int na, int nu, int nv, bool raw, int &u0,
                                            int &v0, int &w, int &h)
 {
-    const float c0 = fmaxf((float)P - 0.5f, 0.0f), c1 = fminf((float)P + 1.5f, (float)na);
+    // plane P serves base indices P - 1 and P; the outer base indices also own the outer half voxel (clamp to edge)
+    const float c0 = P <= 1 ? 0.0f : (float)P - 0.5f, c1 = P >= na - 2 ? (float)na : (float)P + 1.5f;
     float umin = 3.0e38f, umax = -3.0e38f, vmin = 3.0e38f, vmax = -3.0e38f;
     for (int k = 0; k < 4; ++k) {
         const float ua = fmaf(c0, L[k].Ru, L[k].Au), ub = fmaf(c1, L[k].Ru, L[k].Au);
@@ -90,6 +92,22 @@ __host__ __device__ inline void plane_rect(const BeamLine L[4], int P, int na, i
     }
     u0 = iu0; v0 = iv0;
     w = iu1 - iu0 + 2; h = iv1 - iv0 + 2;
+}
+
+// Largest raw plane rectangle over the planes [Pa, Pb] of a beam, up to one voxel: the raw size is convex in the
+// plane index over the interior planes (all serve a 2-voxel range) but not across the two outer planes at
+// either volume face (they serve the outer half voxel too), so the three planes at each end are evaluated
+// (tests/geom_check.cu checks the bound by brute force).
+__host__ __device__ inline void beam_rect_bound(const BeamLine L[4], int Pa, int Pb, int na, int nu, int nv, int &w, int &h)
+{
+    w = 0; h = 0;
+    for (int e = 0; e < 6; ++e) {
+        const int P = e < 3 ? Pa + e : Pb - (e - 3);
+        if (P < Pa || P > Pb) continue;
+        int u0, v0, wp, hp;
+        plane_rect(L, P, na, nu, nv, true, u0, v0, wp, hp);
+        w = wp > w ? wp : w; h = hp > h ? hp : h;
+    }
 }
 
 }  // namespace vr

@@ -468,12 +468,10 @@ k_shear(CamK cam, VolK V, TfK tf, ShearPlanK P, float *__restrict__ image, long 
             BeamLine L[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) L[k] = B.lines[k];
-            // the rectangle must fit at both ends of the beam (its raw size is convex in the plane index)
-            int u0, v0, w0, h0, w1, h1;
-            plane_rect(L, B.iw_min, B.na, B.nu, B.nv, true, u0, v0, w0, h0);
-            plane_rect(L, B.iw_max + 1, B.na, B.nu, B.nv, true, u0, v0, w1, h1);
-            // (+ 1: the floors make the size convex only up to one voxel)
-            ok = min(max(w0, w1) + 1, B.nu) <= B.PU && min(max(h0, h1) + 1, B.nv) <= B.PV;
+            // every plane of the beam must fit a slot: beam_rect_bound() is their largest raw size up to one voxel
+            int wb, hb;
+            beam_rect_bound(L, B.iw_min, B.iw_max + 1, B.na, B.nu, B.nv, wb, hb);
+            ok = min(wb + 1, B.nu) <= B.PU && min(hb + 1, B.nv) <= B.PV;
         }
         if (!ok) { if (lane == 0) { ctl[kCtlDirect] = 1; atomicAdd(P.overflow + 1, 1u); } }
         else { plan_step(B, 0, true, next_ord, wstart); plan_step(B, 1, false, next_ord, wstart); }
@@ -547,14 +545,13 @@ void plan_caps(const CamK &cam, const int n[3], int tiles_x, int tiles_y, int ca
                 if (hi >= lo) { c_lo = std::min(c_lo, lo); c_hi = std::max(c_hi, hi); }
             }
             if (!valid || c_hi < c_lo) continue;            // marched from global memory / misses the volume
-            const int P0 = std::max(0, (int)std::floor(c_lo) - 1), P1 = std::min(n[a], (int)std::ceil(c_hi) + 1);
-            int u0, v0, w0, h0, w1, h1;
-            plane_rect(L, P0, n[a], n[u], n[v], true, u0, v0, w0, h0);
-            plane_rect(L, P1, n[a], n[u], n[v], true, u0, v0, w1, h1);
+            const int P0 = std::max(0, (int)std::floor(c_lo) - 1), P1 = std::min(n[a] - 1, (int)std::ceil(c_hi) + 1);
+            int wb, hb;
+            beam_rect_bound(L, P0, P1, n[a], n[u], n[v], wb, hb);
             // + 2: the kernel tests the planes at the ends of the beam's own sample range (the floors let the
             // size differ by one between neighbouring planes) and asks for one voxel to spare
-            cap[a][0] = std::max(cap[a][0], std::min(std::max(w0, w1) + 2, n[u]));
-            cap[a][1] = std::max(cap[a][1], std::min(std::max(h0, h1) + 2, n[v]));
+            cap[a][0] = std::max(cap[a][0], std::min(wb + 2, n[u]));
+            cap[a][1] = std::max(cap[a][1], std::min(hb + 2, n[v]));
         }
 }
 
