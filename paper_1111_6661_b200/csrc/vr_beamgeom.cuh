@@ -110,4 +110,34 @@ __host__ __device__ inline void beam_rect_bound(const BeamLine L[4], int Pa, int
     }
 }
 
+// ---------------------------------------------------------------- step schedule of the sheared-plane path
+// (vr_shear.cu; also executed on the host by the schedule model of tests/geom_check.cu).  The data planes of a
+// beam, iw_min .. iw_max + 1, are numbered by their ordinal j along the direction of travel; base plane ordinal
+// jb needs data ordinals jb and jb + 1.  Step 0 loads G + 1 planes, every later step G; after the planes up to
+// ordinal m have landed the base ordinals below m can be marched.  Plane ordinal j lives in ring slot j mod NS.
+struct StepPlan { int nload, wlo, wn; };       // planes to load before the step; base planes [wlo, wlo + wn) it marches
+
+__host__ __device__ inline int plane_of_ordinal(int sgn, int iw_min, int iw_max, int j)
+{
+    return sgn > 0 ? iw_min + j : iw_max + 1 - j;
+}
+__host__ __device__ inline int ring_slot(int j, int NS) { return j % NS; }
+
+// next step of the schedule; next_ord = first plane ordinal not yet planned, wstart = first base ordinal not yet marched
+__host__ __device__ inline StepPlan plan_window(bool first, int G, int sgn, int iw_min, int iw_max, int &next_ord, int &wstart)
+{
+    const int n_planes = iw_max - iw_min + 2;
+    int nload = first ? G + 1 : G;
+    if (nload > n_planes - next_ord) nload = n_planes - next_ord;
+    if (nload < 0) nload = 0;
+    next_ord += nload;
+    const int wend = next_ord - 1 > wstart ? next_ord - 1 : wstart;
+    StepPlan S;
+    S.nload = nload;
+    S.wlo = sgn > 0 ? iw_min + wstart : iw_max - wend + 1;
+    S.wn = wend - wstart;
+    wstart = wend;
+    return S;
+}
+
 }  // namespace vr

@@ -197,22 +197,22 @@ struct BeamCtx {
 __device__ __forceinline__ void plan_step(const BeamCtx &B, int rec, bool first, int &next_ord, int &wstart)
 {
     const int lane = threadIdx.x & 31;
-    const int n_planes = B.iw_max - B.iw_min + 2;
-    const int nload = max(min(first ? B.G + 1 : B.G, n_planes - next_ord), 0);
+    const int ord0 = next_ord;
+    const StepPlan S = plan_window(first, B.G, B.sgn, B.iw_min, B.iw_max, next_ord, wstart);
     BeamLine L[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) L[k] = B.lines[k];
     int w = 0, h = 0;
-    if (lane < nload) {
-        const int j = next_ord + lane;
-        const int q = B.sgn > 0 ? B.iw_min + j : B.iw_max + 1 - j;
+    if (lane < S.nload) {
+        const int j = ord0 + lane;
+        const int q = plane_of_ordinal(B.sgn, B.iw_min, B.iw_max, j);
         int u0, v0;
         plane_rect(L, q, B.na, B.nu, B.nv, false, u0, v0, w, h);
-        if (w > B.PU || h > B.PV) {                                   // never expected (fit test at both beam ends)
+        if (w > B.PU || h > B.PV) {                                   // never expected (fit test over the beam's planes)
             *reinterpret_cast<volatile unsigned int *>(B.overflow) = 1u;
             w = min(w, B.PU); h = min(h, B.PV);
         }
-        const unsigned int sdst = B.buf_a + 4u * (unsigned int)((j % B.NS) * B.PP);
+        const unsigned int sdst = B.buf_a + 4u * (unsigned int)(ring_slot(j, B.NS) * B.PP);
         const unsigned int tv = sdst - 4u * (unsigned int)(u0 + v0 * B.PU);
         B.tab[q & 63] = tv; B.tab[(q & 63) + 64] = tv;
         LoadRec &R = B.loads[rec * 20 + lane];
@@ -220,14 +220,10 @@ __device__ __forceinline__ void plan_step(const BeamCtx &B, int rec, bool first,
         R.g0 = B.vbase + ((long long)q * B.sq + (long long)u0 * B.su + (long long)v0 * B.sv);
     }
     const int wmax = __reduce_max_sync(0xffffffffu, w), hmax = __reduce_max_sync(0xffffffffu, h);
-    next_ord += nload;
-    const int wend = max(next_ord - 1, wstart);
     if (lane == 0) {
-        StepRec &S = B.steps[rec];
-        S.wlo = B.sgn > 0 ? B.iw_min + wstart : B.iw_max - wend + 1;
-        S.wn = wend - wstart; S.nload = nload; S.wmax = wmax; S.hmax = hmax;
+        StepRec &R = B.steps[rec];
+        R.wlo = S.wlo; R.wn = S.wn; R.nload = S.nload; R.wmax = wmax; R.hmax = hmax;
     }
-    wstart = wend;
 }
 
 // all warps: enqueue the cp.async copies of the load list of step record `rec`.

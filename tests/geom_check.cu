@@ -1,11 +1,13 @@
 // geom_check.cu — brute-force check of the beam geometry of vr_beamgeom.cuh on the HOST (no GPU): for random
 // cameras, volumes and beams, every sample position a ray of the beam can take must read only voxels inside
-// plane_rect() of the two data planes it touches (a voxel outside would be read from stale shared memory).
+// plane_rect() of the two data planes it touches (a voxel outside would be read from stale shared memory); and a
+// host model of the kernel's step loop runs the kernel's own schedule functions over random beams.
 // Built and run by tests/test_beam_geometry.py (nvcc compiles it as host code).  Test infrastructure.
 #include <cstdio>
 #include <cstdlib>
 #include <cmath>
 #include <random>
+#include <vector>
 
 #include "../paper_1111_6661_b200/csrc/vr_beamgeom.cuh"
 
@@ -16,6 +18,60 @@ static void cross(const double a[3], const double b[3], double c[3])
     c[0] = a[1] * b[2] - a[2] * b[1]; c[1] = a[2] * b[0] - a[0] * b[2]; c[2] = a[0] * b[1] - a[1] * b[0];
 }
 static void norm(double a[3]) { double l = std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); for (int i = 0; i < 3; ++i) a[i] /= l; }
+
+// Host model of the step loop of run_beam() in vr_shear.cu, executing the SAME plan_window() / ring_slot() /
+// plane_of_ordinal(): loads of step s + 1 are in flight while step s marches, the planner writes the address
+// table two steps ahead.  Checks: every base plane is marched exactly once, in travel order; both data planes of
+// a marched base plane are resident in a ring slot that no in-flight copy may overwrite; the 64-entry address
+// table still points at them.
+static long long check_schedule(std::mt19937_64 &rng, long long &bad)
+{
+    std::uniform_real_distribution<double> U(0.0, 1.0);
+    const int iw_min = (int)(U(rng) * 300), iw_max = iw_min + (int)(U(rng) * (U(rng) < 0.3 ? 3 : 400));
+    const int sgn = U(rng) < 0.5 ? 1 : -1, G = 1 + (int)(U(rng) * 16), NS = 2 * G + 1 + (U(rng) < 0.3 ? (int)(U(rng) * 4) : 0);
+    const int n_base = iw_max - iw_min + 1;
+    int next_ord = 0, wstart = 0, ord0[3];
+    StepPlan rec[3];
+    std::vector<int> ring(NS, -1), covered(n_base, 0);
+    int tab[64];
+    for (int i = 0; i < 64; ++i) tab[i] = -1;
+    auto ordinal = [&](int q) { return sgn > 0 ? q - iw_min : iw_max + 1 - q; };
+    auto plan = [&](int r, bool first) {
+        ord0[r] = next_ord;
+        rec[r] = plan_window(first, G, sgn, iw_min, iw_max, next_ord, wstart);
+        for (int k = 0; k < rec[r].nload; ++k) { const int q = plane_of_ordinal(sgn, iw_min, iw_max, ord0[r] + k); tab[q & 63] = q; }
+    };
+    auto land = [&](int r) {
+        for (int k = 0; k < rec[r].nload; ++k) ring[ring_slot(ord0[r] + k, NS)] = plane_of_ordinal(sgn, iw_min, iw_max, ord0[r] + k);
+    };
+    plan(0, true); plan(1, false);
+    land(0);
+    long long n = 0;
+    int last = sgn > 0 ? iw_min - 1 : iw_max + 1;
+    for (int it = 0;; ++it) {
+        const StepPlan S = rec[it % 3];
+        if (S.wn == 0) break;
+        std::vector<char> inflight(NS, 0);
+        const int r1 = (it + 1) % 3;
+        for (int k = 0; k < rec[r1].nload; ++k) inflight[ring_slot(ord0[r1] + k, NS)] = 1;
+        plan((it + 2) % 3, false);
+        for (int t = 0; t < S.wn; ++t) {
+            const int ia = sgn > 0 ? S.wlo + t : S.wlo + S.wn - 1 - t;            // travel order inside the window
+            if (ia < iw_min || ia > iw_max) { ++bad; continue; }
+            if (ia != last + sgn) ++bad;
+            last = ia;
+            covered[ia - iw_min]++;
+            for (int q = ia; q <= ia + 1; ++q) {
+                const int slot = ring_slot(ordinal(q), NS);
+                if (ring[slot] != q || inflight[slot] || tab[q & 63] != q) ++bad;
+                ++n;
+            }
+        }
+        land(r1);
+    }
+    for (int c : covered) if (c != 1) ++bad;
+    return n;
+}
 
 int main(int argc, char **argv)
 {
@@ -99,6 +155,9 @@ int main(int argc, char **argv)
                 }
             }
     }
-    printf("beams %lld skipped %lld checked %lld rect_bad %lld convex_bad %lld\n", beams, skipped, checked, rect_bad, convex_bad);
-    return (rect_bad || convex_bad || checked < 100000) ? 1 : 0;
+    long long sched_bad = 0, sched_checked = 0;
+    for (int k = 0; k < 20000; ++k) sched_checked += check_schedule(rng, sched_bad);
+    printf("beams %lld skipped %lld checked %lld rect_bad %lld convex_bad %lld schedule_checked %lld schedule_bad %lld\n", beams,
+           skipped, checked, rect_bad, convex_bad, sched_checked, sched_bad);
+    return (rect_bad || convex_bad || sched_bad || checked < 100000 || sched_checked < 100000) ? 1 : 0;
 }
