@@ -11,6 +11,7 @@
 #include <new>
 
 #include "vr_internal.h"
+#include "vr_plan.h"
 
 namespace vr {
 
@@ -221,50 +222,6 @@ static vr_status stream_brick_release(vr_volume *v, uint32_t slot, cudaStream_t 
 // ------------------------------------------------------------------ per-frame brick planning (A4)
 struct PlannedBrick { BrickK k; double key; uint32_t b[3]; uint64_t id; };
 
-static bool zero3(const float *a) { return a[0] == 0.0f && a[1] == 0.0f && a[2] == 0.0f; }
-
-static double det3(const double a[3], const double b[3], const double c[3])
-{
-    return a[0] * (b[1] * c[2] - b[2] * c[1]) - b[0] * (a[1] * c[2] - a[2] * c[1]) + c[0] * (a[1] * b[2] - a[2] * b[1]);
-}
-
-// conservative screen rectangle of an axis-aligned box of sample positions
-static void box_rect(const vr_camera *c, bool perspective, const double lo[3], const double hi[3], int &x0, int &y0,
-                     int &x1, int &y1)
-{
-    const int W = (int)c->width, H = (int)c->height;
-    double mnx = 1e300, mny = 1e300, mxx = -1e300, mxy = -1e300;
-    bool full = false;
-    for (int corner = 0; corner < 8 && !full; ++corner) {
-        double P[3];
-        for (int a = 0; a < 3; ++a) P[a] = (corner >> a & 1) ? hi[a] : lo[a];
-        double x, y;
-        if (perspective) {            // d0 + x du + y dv = lambda (P - o0)
-            double m0[3], m1[3], m2[3], rhs[3];
-            for (int a = 0; a < 3; ++a) { m0[a] = c->du[a]; m1[a] = c->dv[a]; m2[a] = -(P[a] - (double)c->o0[a]); rhs[a] = -(double)c->d0[a]; }
-            const double D = det3(m0, m1, m2);
-            if (std::fabs(D) < 1e-300) { full = true; break; }
-            x = det3(rhs, m1, m2) / D; y = det3(m0, rhs, m2) / D;
-            const double lambda = det3(m0, m1, rhs) / D;
-            if (!(lambda > 1e-9)) { full = true; break; }       // corner at or behind the eye
-        } else {                      // o0 + x ou + y ov + t d0 = P
-            double m0[3], m1[3], m2[3], rhs[3];
-            for (int a = 0; a < 3; ++a) { m0[a] = c->ou[a]; m1[a] = c->ov[a]; m2[a] = c->d0[a]; rhs[a] = P[a] - (double)c->o0[a]; }
-            const double D = det3(m0, m1, m2);
-            if (std::fabs(D) < 1e-300) { full = true; break; }
-            x = det3(rhs, m1, m2) / D; y = det3(m0, rhs, m2) / D;
-        }
-        if (!std::isfinite(x) || !std::isfinite(y)) { full = true; break; }
-        mnx = std::min(mnx, x); mxx = std::max(mxx, x); mny = std::min(mny, y); mxy = std::max(mxy, y);
-    }
-    if (full) { x0 = 0; y0 = 0; x1 = W; y1 = H; return; }
-    // pixel i has x = i + 0.5; one extra pixel of slack for float32 ray arithmetic
-    const double fx0 = std::floor(mnx - 0.5) - 1.0, fy0 = std::floor(mny - 0.5) - 1.0;
-    const double fx1 = std::ceil(mxx - 0.5) + 2.0, fy1 = std::ceil(mxy - 0.5) + 2.0;
-    x0 = (int)std::min(std::max(fx0, 0.0), (double)W); x1 = (int)std::min(std::max(fx1, 0.0), (double)W);
-    y0 = (int)std::min(std::max(fy0, 0.0), (double)H); y1 = (int)std::min(std::max(fy1, 0.0), (double)H);
-}
-
 // bricks that own samples and touch the screen, in visibility order (C.7)
 static void plan_bricks(const vr_volume *v, const vr_camera *c, std::vector<PlannedBrick> &out, uint32_t &culled)
 {
@@ -283,12 +240,8 @@ static void plan_bricks(const vr_volume *v, const vr_camera *c, std::vector<Plan
                 for (int a = 0; a < 3; ++a) {
                     owned_range(v, a, p.b[a], p.k.lo[a], p.k.hi[a]);
                     if (p.k.lo[a] > p.k.hi[a]) empty = true;
-                    // ownership cell in position space, outer cells reach the volume faces; 0.01 voxel slack
-                    lo[a] = (p.k.lo[a] == 0 ? 0.0 : p.k.lo[a] + 0.5) - 0.01;
-                    hi[a] = (p.k.hi[a] == n[a] - 2 ? (double)n[a] : p.k.hi[a] + 1.5) + 0.01;
-                    const double centre = (double)v->B * (p.b[a] + 0.5) + 0.5;      // ownership-lattice centre
-                    if (perspective) { const double e = (double)c->o0[a] - centre; p.key += e * e; }
-                    else p.key += centre * (double)c->d0[a];
+                    brick_cell(p.k.lo[a], p.k.hi[a], n[a], lo[a], hi[a]);
+                    p.key += brick_key_term(perspective, (double)v->B, p.b[a], (double)c->o0[a], (double)c->d0[a]);
                 }
                 if (empty) continue;
                 box_rect(c, perspective, lo, hi, p.k.x0, p.k.y0, p.k.x1, p.k.y1);
