@@ -110,6 +110,37 @@ __host__ __device__ inline void beam_rect_bound(const BeamLine L[4], int Pa, int
     }
 }
 
+// Range [c_lo, c_hi] of the principal coordinate over which the cross-section of the beam (the quadrilateral of
+// its four corner lines) can overlap the volume: the hull of all c in [0, na] at which the bounding box of the
+// four corner points overlaps [0,nu] x [0,nv].  Conservative on purpose — a beam that straddles a volume edge
+// or contains the whole volume has rays inside the volume although none of its corner lines is.  The feasible
+// set changes only where a corner line crosses a face plane, so its ends are among those crossings, 0 and na.
+// false: no overlap at all.
+__host__ __device__ inline bool beam_c_range(const BeamLine L[4], int na, int nu, int nv, float &c_lo, float &c_hi)
+{
+    float cand[18];
+    int nc = 0;
+    cand[nc++] = 0.0f; cand[nc++] = (float)na;
+    for (int k = 0; k < 4; ++k) {
+        if (L[k].Ru != 0.0f) { cand[nc++] = (0.0f - L[k].Au) / L[k].Ru; cand[nc++] = ((float)nu - L[k].Au) / L[k].Ru; }
+        if (L[k].Rv != 0.0f) { cand[nc++] = (0.0f - L[k].Av) / L[k].Rv; cand[nc++] = ((float)nv - L[k].Av) / L[k].Rv; }
+    }
+    c_lo = 3.0e38f; c_hi = -3.0e38f;
+    for (int i = 0; i < nc; ++i) {
+        const float c = fminf(fmaxf(cand[i], 0.0f), (float)na);
+        float umin = 3.0e38f, umax = -3.0e38f, vmin = 3.0e38f, vmax = -3.0e38f;
+        for (int k = 0; k < 4; ++k) {
+            const float u = fmaf(c, L[k].Ru, L[k].Au), v = fmaf(c, L[k].Rv, L[k].Av);
+            umin = fminf(umin, u); umax = fmaxf(umax, u); vmin = fminf(vmin, v); vmax = fmaxf(vmax, v);
+        }
+        // one voxel of slack: the candidates are the exact boundaries of the feasible set
+        if (umin <= (float)nu + 1.0f && umax >= -1.0f && vmin <= (float)nv + 1.0f && vmax >= -1.0f) {
+            c_lo = fminf(c_lo, c); c_hi = fmaxf(c_hi, c);
+        }
+    }
+    return c_hi >= c_lo;
+}
+
 // ---------------------------------------------------------------- step schedule of the sheared-plane path
 // (vr_shear.cu; also executed on the host by the schedule model of tests/geom_check.cu).  The data planes of a
 // beam, iw_min .. iw_max + 1, are numbered by their ordinal j along the direction of travel; base plane ordinal

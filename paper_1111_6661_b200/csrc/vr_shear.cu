@@ -501,8 +501,8 @@ k_shear(CamK cam, VolK V, TfK tf, ShearPlanK P, float *__restrict__ image, long 
 }
 
 // ------------------------------------------------------------------ host: per-frame plan
-// Largest plane rectangle per principal-axis class over a sample of the frame's beams (every beam when there
-// are few, a regular sub-grid plus the image border otherwise).  The raw rectangle size is convex in the plane
+// Largest plane rectangle per principal-axis class over the frame's beams (every beam up to 65536 beams — all of
+// the five configs —, a regular sub-grid plus the image border beyond).  The raw rectangle size is convex in the plane
 // index, so per beam it is evaluated at the two ends of the part of the beam inside the volume.  A sizing
 // heuristic, not a guarantee: the kernel marches a beam whose planes do not fit from global memory, so an
 // under-estimate costs time, never correctness.  cap[a][0] == 0: no sampled beam of class a.
@@ -510,7 +510,7 @@ void plan_caps(const CamK &cam, const int n[3], int tiles_x, int tiles_y, int ca
 {
     for (int a = 0; a < 3; ++a) cap[a][0] = cap[a][1] = 0;
     const int W = cam.width, H = cam.height;
-    const int stride = std::max(1, (int)std::ceil(std::sqrt((double)tiles_x * tiles_y / 4096.0)));
+    const int stride = std::max(1, (int)std::ceil(std::sqrt((double)tiles_x * tiles_y / 65536.0)));
     for (int ty = 0; ty < tiles_y; ++ty)
         for (int tx = 0; tx < tiles_x; ++tx) {
             const bool border = tx == 0 || ty == 0 || tx == tiles_x - 1 || ty == tiles_y - 1;
@@ -524,23 +524,12 @@ void plan_caps(const CamK &cam, const int n[3], int tiles_x, int tiles_y, int ca
             beam_axes(a, u, v);
             BeamLine L[4];
             bool valid = true;
-            float c_lo = 1e30f, c_hi = -1e30f;
             for (int c = 0; c < 4 && valid; ++c) {
                 const float cx = (float)((c & 1) ? std::min(x0 + kBW, W) : x0), cy = (float)((c & 2) ? std::min(y0 + kBH, H) : y0);
-                if (!beam_line(cam, cx, cy, a, sgn, L[c])) { valid = false; break; }
-                // the part of this corner line inside the volume, as an interval of the principal coordinate
-                float lo = 0.0f, hi = (float)n[a];
-                const float A2[2] = { L[c].Au, L[c].Av }, R2[2] = { L[c].Ru, L[c].Rv };
-                const int ax[2] = { u, v };
-                for (int e = 0; e < 2; ++e) {
-                    if (R2[e] != 0.0f) {
-                        const float c0 = (0.0f - A2[e]) / R2[e], c1 = ((float)n[ax[e]] - A2[e]) / R2[e];
-                        lo = std::max(lo, std::min(c0, c1)); hi = std::min(hi, std::max(c0, c1));
-                    } else if (A2[e] < 0.0f || A2[e] > (float)n[ax[e]]) hi = -1e30f;
-                }
-                if (hi >= lo) { c_lo = std::min(c_lo, lo); c_hi = std::max(c_hi, hi); }
+                valid = beam_line(cam, cx, cy, a, sgn, L[c]);
             }
-            if (!valid || c_hi < c_lo) continue;            // marched from global memory / misses the volume
+            float c_lo, c_hi;
+            if (!valid || !beam_c_range(L, n[a], n[u], n[v], c_lo, c_hi)) continue;   // marched from global memory / misses the volume
             const int P0 = std::max(0, (int)std::floor(c_lo) - 1), P1 = std::min(n[a] - 1, (int)std::ceil(c_hi) + 1);
             int wb, hb;
             beam_rect_bound(L, P0, P1, n[a], n[u], n[v], wb, hb);
@@ -551,27 +540,22 @@ void plan_caps(const CamK &cam, const int n[3], int tiles_x, int tiles_y, int ca
         }
 }
 
-}  // namespace
-
-// Enqueues one frame.  *applied = false (and VR_OK) if nothing was enqueued because not even three plane slots
-// fit shared memory (the caller then uses another path).
-vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, const VolK &V, const TfK &tf,
-                       unsigned int *overflow_dev, float *image, long long pitch_f, cudaStream_t st, bool *applied)
+// The per-frame plan of k_shear: slot size per principal-axis class, planes per step, ring slots, shared memory.
+// Pure host arithmetic on the camera and the volume dims (tests/shear_plan_check.cu runs it without a GPU).
+// false: not even three plane slots fit shared memory.
+bool make_shear_plan(bool sparse_direct, const CamK &cam, const int n[3], unsigned int *overflow_dev, ShearPlanK &P,
+                     unsigned int &smem_bytes)
 {
-    *applied = false;
-    const int n[3] = { V.nx, V.ny, V.nz };
     const int W = cam.width, H = cam.height;
     const int tiles_x = (W + kBW - 1) / kBW, tiles_y = (H + kBH - 1) / kBH;
-    if ((long long)tiles_x * tiles_y > 0x7fffffffll) return VR_OK;
-
-    ShearPlanK P;
     memset(&P, 0, sizeof(P));
     P.tiles_x = tiles_x; P.tiles_y = tiles_y; P.overflow = overflow_dev;
     int cap[3][2];
     plan_caps(cam, n, tiles_x, tiles_y, cap);
     // Per class: the ring of 2 G + 1 plane slots with the largest G that leaves room for three CTAs per SM
     // (if G >= 3), else for two (G >= 2), else for one; else shrink the slots (beams that then do not fit
-    // march from global memory).  Class 0 loads with G + 1 lanes per cell, so there G + 1 is a power of two.
+    // march from global memory).  (Class 0 loads with 2^ceil(log2(planes)) lanes per cell; any G works, G + 1 or G
+    // a power of two wastes no lanes.)
     // VR_OPT_SPARSE_DIRECT (experimental, off by default; not yet measured end to end).  Sparse sampling (cfg4:
     // 1.7-3.3 voxels per pixel, step 1): neighbouring rays share no voxel, so staging a whole plane rectangle
     // moves cap_w * cap_h / 256 words per ray and plane for the 8 a ray reads.  Measured on cfg4 with the
@@ -606,8 +590,7 @@ vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, 
             for (int a = 0; a < 3; ++a) {
                 if (cap[a][0] == 0) { P.G[a] = 1; P.NS[a] = 3; continue; }         // class not in this frame
                 const int ns = (int)std::min<unsigned int>(budget / (unsigned int)P.PP[a], 2u * (kMaxLoad - 1) + 1u);
-                int g = (ns - 1) / 2;
-                if (a == 0) g = g >= 15 ? 15 : g >= 7 ? 7 : g >= 3 ? 3 : g >= 1 ? 1 : 0;
+                const int g = (ns - 1) / 2;
                 if (g < g_min) { fits = false; break; }
                 P.G[a] = g; P.NS[a] = 2 * g + 1;
                 ring_words = std::max(ring_words, (unsigned int)P.NS[a] * (unsigned int)P.PP[a]);
@@ -622,11 +605,27 @@ vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, 
         fprintf(stderr, "shear: class %d G %d NS %d PU %d PV %d PP %d\n", a, P.G[a], P.NS[a], P.PU[a], P.PV[a], P.PP[a]);
     fprintf(stderr, "fits %d ring_words %u\n", (int)fits, ring_words);
 #endif
-    if (!fits) return VR_OK;
+    if (!fits) return false;
     for (int a = 0; a < 3; ++a)                                                      // unused classes: still addressable
         ring_words = std::max(ring_words, (unsigned int)P.NS[a] * (unsigned int)P.PP[a]);
-    const unsigned int smem_bytes = kBufOff + 4u * ring_words;
-    if (smem_bytes > kSmemMax) return VR_OK;
+    smem_bytes = kBufOff + 4u * ring_words;
+    return smem_bytes <= kSmemMax;
+}
+
+}  // namespace
+
+// Enqueues one frame.  *applied = false (and VR_OK) if nothing was enqueued because not even three plane slots
+// fit shared memory (the caller then uses another path).
+vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, const VolK &V, const TfK &tf,
+                       unsigned int *overflow_dev, float *image, long long pitch_f, cudaStream_t st, bool *applied)
+{
+    *applied = false;
+    const int n[3] = { V.nx, V.ny, V.nz };
+    const int tiles_x = (cam.width + kBW - 1) / kBW, tiles_y = (cam.height + kBH - 1) / kBH;
+    if ((long long)tiles_x * tiles_y > 0x7fffffffll) return VR_OK;
+    ShearPlanK P;
+    unsigned int smem_bytes = 0;
+    if (!make_shear_plan(sparse_direct, cam, n, overflow_dev, P, smem_bytes)) return VR_OK;
 
     const int grid = tiles_x * tiles_y;
 #define VR_SHEAR_LAUNCH(M, E)                                                                                         \
