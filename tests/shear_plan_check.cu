@@ -74,6 +74,7 @@ int main(int argc, char **argv)
         unsigned int smem = 0;
         const bool fits = make_shear_plan(false, cam, n, nullptr, P, smem);
         long long beams = 0, direct_fit = 0, direct_oblique = 0, overflow = 0;
+        double staged = 0.0;                        // bytes the frame copies into shared memory
         for (int ty = 0; fits && ty * kBH < H; ++ty)
             for (int tx = 0; tx * kBW < W; ++tx) {
                 const int x0 = tx * kBW, y0 = ty * kBH;
@@ -104,12 +105,13 @@ int main(int argc, char **argv)
                     int u0, v0, w, h;
                     plane_rect(L, q, n[a], n[au], n[av], false, u0, v0, w, h);
                     if (w > P.PU[a] || h > P.PV[a]) ++overflow;
+                    staged += 4.0 * w * h;
                 }
             }
         const int ctas = std::min(3, (int)(kSmemSM / (smem + 1024u)));
-        printf("view %d: %dx%dx%d %dx%d fits %d smem %u ctas %d | x: PU %d PV %d G %d | y: PU %d PV %d G %d | z: PU %d PV %d G %d | beams %lld direct_fit %lld direct_oblique %lld overflow %lld\n",
+        printf("view %d: %dx%dx%d %dx%d fits %d smem %u ctas %d | x: PU %d PV %d G %d | y: PU %d PV %d G %d | z: PU %d PV %d G %d | beams %lld direct_fit %lld direct_oblique %lld overflow %lld staged %.2f GB = %.2f x volume\n",
                view, n[0], n[1], n[2], W, H, (int)fits, smem, ctas, P.PU[0], P.PV[0], P.G[0], P.PU[1], P.PV[1], P.G[1], P.PU[2], P.PV[2], P.G[2],
-               beams, direct_fit, direct_oblique, overflow);
+               beams, direct_fit, direct_oblique, overflow, staged / 1e9, staged / (4.0 * n[0] * n[1] * n[2]));
         for (int a = 0; a < 3 && fits; ++a)
             if (P.NS[a] < 2 * P.G[a] + 1 || P.G[a] + 1 > kMaxLoad || 3 * P.G[a] + 1 > 64 || P.PP[a] < P.PU[a] * P.PV[a] || smem > kSmemMax) ++overflow;
         tot_direct += direct_fit; tot_overflow += overflow; tot_beams += beams;
