@@ -14,7 +14,7 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
     "--fmad=false",                 # nothing is contracted behind the canonical arithmetic's back
-    "-Xcompiler", "-fPIC,-fvisibility=hidden,-O2",
+    "-Xcompiler", "-fPIC,-fvisibility=hidden,-O2,-mfma,-ffp-contract=off",   # fmaf inlined in the host plans, nothing contracted implicitly
     "-shared", "-cudart", "static",
 ]
 

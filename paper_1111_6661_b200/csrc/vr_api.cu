@@ -105,6 +105,7 @@ struct vr_volume {
     unsigned int tile_serial = 0;
     uint64_t tile_done_sig = 0;               // tile grid the done flags were cleared for
     int opt_path = 0, opt_tile = 0, opt_sparse = 0;   // vr_set_option
+    ShearPlanCache *shear_cache = nullptr;    // last per-frame plans of the sheared-plane path
     unsigned int *beam_overflow_h = nullptr;  // mapped pinned words: [0] set if a staged box / plane overflowed, [1] beams marched from global memory
     unsigned int *beam_overflow_d = nullptr;
     Staging staging[kStagingRing];
@@ -134,6 +135,7 @@ static void free_volume(vr_volume *v)
     if (v->d_sum) cudaFree(v->d_sum);
     if (v->d_sum_out) cudaFree(v->d_sum_out);
     if (v->beam_overflow_h) cudaFreeHost(v->beam_overflow_h);
+    shear_cache_destroy(v->shear_cache);
     v->arena.release();
     v->host_image.release();
     v->tile_work.release(); v->tile_ctrl.release(); v->tile_done.release();
@@ -523,7 +525,7 @@ static vr_status render_shear(vr_volume *v, const CamK &cam, int mode, bool ert,
     VolK V;
     V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
     V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz; V.ox = V.oy = V.oz = 0;
-    vr_status rc = launch_shear(mode, ert, v->opt_sparse != 0, cam, V, tf, v->beam_overflow_d, img, pitch_f, st, applied);
+    vr_status rc = launch_shear(mode, ert, v->opt_sparse != 0, cam, V, tf, v->beam_overflow_d, v->shear_cache, img, pitch_f, st, applied);
     if (rc != VR_OK || !*applied) return rc;
     v->stats.kernel_launches += 1;
     v->stats.path = 6;
@@ -624,6 +626,7 @@ VR_API vr_status vr_create_volume(const vr_volume_desc *d, vr_volume **out)
     VR_FAIL_CUDA(cudaHostAlloc(&v->beam_overflow_h, 2 * sizeof(unsigned int), cudaHostAllocMapped));
     v->beam_overflow_h[0] = v->beam_overflow_h[1] = 0u;
     VR_FAIL_CUDA(cudaHostGetDevicePointer(&v->beam_overflow_d, v->beam_overflow_h, 0));
+    v->shear_cache = shear_cache_create();       // nullptr (allocation failure) only means no caching
 #undef VR_FAIL_CUDA
     *out = v;
     return VR_OK;

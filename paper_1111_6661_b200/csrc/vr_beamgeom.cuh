@@ -111,33 +111,32 @@ __host__ __device__ inline void beam_rect_bound(const BeamLine L[4], int Pa, int
 }
 
 // Range [c_lo, c_hi] of the principal coordinate over which the cross-section of the beam (the quadrilateral of
-// its four corner lines) can overlap the volume: the hull of all c in [0, na] at which the bounding box of the
-// four corner points overlaps [0,nu] x [0,nv].  Conservative on purpose — a beam that straddles a volume edge
-// or contains the whole volume has rays inside the volume although none of its corner lines is.  The feasible
-// set changes only where a corner line crosses a face plane, so its ends are among those crossings, 0 and na.
-// false: no overlap at all.
+// its four corner lines) can overlap the volume: [0, na] minus the c-intervals on which all four corner points
+// lie beyond the same face of the (u,v) rectangle (by more than a voxel).  Conservative on purpose — a beam that
+// straddles a volume edge or contains the whole volume has rays inside the volume although none of its corner
+// lines is.  false: no overlap at all.
 __host__ __device__ inline bool beam_c_range(const BeamLine L[4], int na, int nu, int nv, float &c_lo, float &c_hi)
 {
-    float cand[18];
-    int nc = 0;
-    cand[nc++] = 0.0f; cand[nc++] = (float)na;
-    for (int k = 0; k < 4; ++k) {
-        if (L[k].Ru != 0.0f) { cand[nc++] = (0.0f - L[k].Au) / L[k].Ru; cand[nc++] = ((float)nu - L[k].Au) / L[k].Ru; }
-        if (L[k].Rv != 0.0f) { cand[nc++] = (0.0f - L[k].Av) / L[k].Rv; cand[nc++] = ((float)nv - L[k].Av) / L[k].Rv; }
-    }
-    c_lo = 3.0e38f; c_hi = -3.0e38f;
-    for (int i = 0; i < nc; ++i) {
-        const float c = fminf(fmaxf(cand[i], 0.0f), (float)na);
-        float umin = 3.0e38f, umax = -3.0e38f, vmin = 3.0e38f, vmax = -3.0e38f;
+    // E[i] = open interval of c on which  s * (p_k(c) - bound) > 0  for all four corners k
+    float e_lo[4], e_hi[4];
+    for (int i = 0; i < 4; ++i) {
+        const bool on_u = i < 2, high = (i & 1) != 0;
+        const float bound = high ? (float)(on_u ? nu : nv) + 1.0f : -1.0f, sg = high ? 1.0f : -1.0f;
+        float lo = -3.0e38f, hi = 3.0e38f;
         for (int k = 0; k < 4; ++k) {
-            const float u = fmaf(c, L[k].Ru, L[k].Au), v = fmaf(c, L[k].Rv, L[k].Av);
-            umin = fminf(umin, u); umax = fmaxf(umax, u); vmin = fminf(vmin, v); vmax = fmaxf(vmax, v);
+            const float A = sg * ((on_u ? L[k].Au : L[k].Av) - bound), R = sg * (on_u ? L[k].Ru : L[k].Rv);   // A + R c > 0
+            if (R > 0.0f) lo = fmaxf(lo, -A / R);
+            else if (R < 0.0f) hi = fminf(hi, -A / R);
+            else if (!(A > 0.0f)) { lo = 3.0e38f; hi = -3.0e38f; }
         }
-        // one voxel of slack: the candidates are the exact boundaries of the feasible set
-        if (umin <= (float)nu + 1.0f && umax >= -1.0f && vmin <= (float)nv + 1.0f && vmax >= -1.0f) {
-            c_lo = fminf(c_lo, c); c_hi = fmaxf(c_hi, c);
-        }
+        e_lo[i] = lo; e_hi[i] = hi;
     }
+    c_lo = 0.0f; c_hi = (float)na;
+    for (int pass = 0; pass < 4; ++pass)
+        for (int i = 0; i < 4; ++i) {
+            if (e_lo[i] < e_hi[i] && e_lo[i] <= c_lo && c_lo < e_hi[i]) c_lo = e_hi[i];
+            if (e_lo[i] < e_hi[i] && e_lo[i] < c_hi && c_hi <= e_hi[i]) c_hi = e_lo[i];
+        }
     return c_hi >= c_lo;
 }
 

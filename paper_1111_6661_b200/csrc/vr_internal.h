@@ -138,7 +138,11 @@ vr_status launch_beam(int mode, bool ert, const CamK &cam, const VolK &vol, cons
 // ---------------------------------------------------------------- sheared-plane beam ray casting (vr_shear.cu)
 // Same beams, but every data plane of a slab is staged as its own rectangle at its own origin by 4-byte
 // cp.async into a bank-conflict-aware layout.  *applied = false: nothing was enqueued.
+struct ShearPlanCache;                       // per-handle cache of the per-frame host plans (camera -> plan)
+ShearPlanCache *shear_cache_create();
+void shear_cache_destroy(ShearPlanCache *c);
 vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, const VolK &vol, const TfK &tf,
-                       unsigned int *overflow_dev, float *image, long long pitch_f, cudaStream_t st, bool *applied);
+                       unsigned int *overflow_dev, ShearPlanCache *cache, float *image, long long pitch_f,
+                       cudaStream_t st, bool *applied);
 
 }  // namespace vr

@@ -31,6 +31,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <new>
 #include <vector>
 
 #include "vr_beamgeom.cuh"
@@ -614,10 +615,21 @@ bool make_shear_plan(bool sparse_direct, const CamK &cam, const int n[3], unsign
 
 }  // namespace
 
+// The plan depends only on the camera, the volume dims and the option: a handle keeps the last plans, so an orbit
+// that is rendered again (or a still camera) pays the host arithmetic (cfg2: ~2 ms, cfg4: ~12 ms) once.
+struct ShearPlanCache {
+    struct Entry { CamK cam; int n[3]; int sparse; ShearPlanK P; unsigned int smem_bytes; int fits; unsigned long long stamp; };
+    std::vector<Entry> e;
+    unsigned long long clock = 0;
+};
+ShearPlanCache *shear_cache_create() { return new (std::nothrow) ShearPlanCache(); }
+void shear_cache_destroy(ShearPlanCache *c) { delete c; }
+
 // Enqueues one frame.  *applied = false (and VR_OK) if nothing was enqueued because not even three plane slots
 // fit shared memory (the caller then uses another path).
 vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, const VolK &V, const TfK &tf,
-                       unsigned int *overflow_dev, float *image, long long pitch_f, cudaStream_t st, bool *applied)
+                       unsigned int *overflow_dev, ShearPlanCache *cache, float *image, long long pitch_f,
+                       cudaStream_t st, bool *applied)
 {
     *applied = false;
     const int n[3] = { V.nx, V.ny, V.nz };
@@ -625,7 +637,27 @@ vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, 
     if ((long long)tiles_x * tiles_y > 0x7fffffffll) return VR_OK;
     ShearPlanK P;
     unsigned int smem_bytes = 0;
-    if (!make_shear_plan(sparse_direct, cam, n, overflow_dev, P, smem_bytes)) return VR_OK;
+    bool fits = false, found = false;
+    if (cache) {
+        for (auto &en : cache->e)
+            if (memcmp(&en.cam, &cam, sizeof(CamK)) == 0 && memcmp(en.n, n, sizeof(n)) == 0 && en.sparse == (int)sparse_direct &&
+                en.P.overflow == overflow_dev) {
+                P = en.P; smem_bytes = en.smem_bytes; fits = en.fits != 0; en.stamp = ++cache->clock; found = true;
+                break;
+            }
+    }
+    if (!found) {
+        fits = make_shear_plan(sparse_direct, cam, n, overflow_dev, P, smem_bytes);
+        if (cache) {
+            ShearPlanCache::Entry en;
+            memset(&en, 0, sizeof(en));
+            en.cam = cam; memcpy(en.n, n, sizeof(n)); en.sparse = (int)sparse_direct; en.P = P; en.smem_bytes = smem_bytes;
+            en.fits = fits ? 1 : 0; en.stamp = ++cache->clock;
+            if (cache->e.size() < 256) cache->e.push_back(en);
+            else *std::min_element(cache->e.begin(), cache->e.end(), [](const ShearPlanCache::Entry &a, const ShearPlanCache::Entry &b) { return a.stamp < b.stamp; }) = en;
+        }
+    }
+    if (!fits) return VR_OK;
 
     const int grid = tiles_x * tiles_y;
 #define VR_SHEAR_LAUNCH(M, E)                                                                                         \
