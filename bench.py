@@ -1,17 +1,19 @@
 #!/usr/bin/env python
 """bench.py — throughput of the hot path on B200, one JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
 
 A *step* is one pass of the whole hot path over one synthetic cube: the data-summary pass
 (vr_minmax_histogram: min/max, then the 256-bin histogram over [min,max]), vr_set_transfer_function
-with that range, and vr_render of every orbit view of the config (for cfg2: 16 perspective views,
-1024x1024, step 0.5, emission-absorption with early ray termination at alpha 0.99).
+with that range, and vr_render of every orbit view of the config.  Default workload: cfg4, the largest
+single-GPU config of BASELINE.json (2048x2048x4096 = 64 GiB resident in HBM, 64 perspective orbit views
+3840x2160, step 1, emission-absorption with early ray termination at alpha 0.99); --config 2|3|5 select
+the others.
 
 value  = nominal voxel samples of all rendered views / step time, cube resident in HBM when the
          timed region starts (CUDA events on the launching stream, max over ranks).
 e2e    = the same metric through the C ABI with HOST buffers: every step creates the handle on the
-         pinned host cube (1 GiB host->device inside the timed region), runs the same calls with
+         pinned host cube (the whole cube host->device inside the timed region), runs the same calls with
          pinned host outputs (summary and images copied device->host) and destroys the handle.
 Multi-GPU: the path does not shard (north_star: one GPU, no collectives) => N independent replicas,
 "scaling": "weak".
@@ -43,6 +45,24 @@ def measured_peaks():
             d = json.load(f)
         return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
     return 6650.0, 1965.0, "fallback"
+
+
+def ncu_traffic(cfg_number: int):
+    """DRAM bytes (read + write) per launch of the ray-march kernel from the committed ncu --set full summary
+    (profiles/ncu_traffic.csv: config,kernel,dram_read_bytes,dram_write_bytes,source), or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    best = None
+    with open(p) as f:
+        for ln in f:
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) >= 4 and c[0] == f"cfg{cfg_number}" and c[1].startswith("k_rows"):
+                try:
+                    best = float(c[2]) + float(c[3])
+                except ValueError:
+                    pass
+    return best
 
 
 # ---------------------------------------------------------------------------------- clocks
@@ -241,7 +261,10 @@ def run_ours(args):
     dev = host.cuda()
     stream = torch.cuda.current_stream()
     modes = modes_of(cfg)
-    cams = [cfg.camera(v) for v in range(cfg.n_views)]
+    view_ids = list(range(cfg.n_views))
+    if args.views > 0:
+        view_ids = view_ids[:: max(1, cfg.n_views // args.views)][: args.views]      # spread over the orbit
+    cams = [cfg.camera(v) for v in view_ids]
     cam_structs = [vr.make_camera(c) for c in cams]
     samples_view = [W.nominal_samples(c, cfg.dims) for c in cams]
     samples_step = sum(samples_view) * len(modes)
@@ -250,6 +273,10 @@ def run_ours(args):
     vol = vr.Volume(dev, cfg.dims, brick=cfg.brick)
     if args.path:
         vol.set_option(vr.VR_OPT_RENDER_PATH, args.path)
+    if args.lag >= 0:
+        vol.set_option(vr.VR_OPT_LANE_LAG, args.lag)
+    if args.no_zcopy:
+        vol.set_option(vr.VR_OPT_ZFAST_COPY, 0)
     sbuf = torch.empty(32 + 8 * 256, dtype=torch.uint8, device="cuda")
     s = vr.Volume.read_summary(vol.minmax_histogram(256, out=sbuf))
     vmin, vmax = float(s["vmin"]), float(s["vmax"])
@@ -297,6 +324,19 @@ def run_ours(args):
     launches = vol.stats()["total_kernel_launches"] - launches0
     render_ms = [a.elapsed_time(b) for a, b in ev_pairs]
     path = vol.stats()["path"]
+    zfast = vol.stats()["zfast_copy"]
+    # cold cameras: one orbit at azimuths none of the steps above has seen (an interactively moving camera);
+    # the per-frame host work of vr_render is O(1) (no per-camera plan, no cache), so this must equal render_ms
+    cold_ms = []
+    if not cfg.sort_last:
+        for v_i in view_ids:
+            c = vr.make_camera(W.orbit_camera(cfg.dims, v_i + 0.37, cfg.n_views, cfg.width, cfg.height, step=cfg.step,
+                                              ert_alpha=cfg.ert_alpha))
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); vol.render(c, modes[0], out=images[modes[0]]); b.record(stream)
+            cold_ms.append((a, b))
+        torch.cuda.synchronize()
+        cold_ms = [a.elapsed_time(b) for a, b in cold_ms]
     ms_total = max_over_ranks([ms_total], dist, "cuda")[0]
     ms_step = ms_total / args.steps
     value = aggregate_value(samples_step, world, ms_step)
@@ -355,7 +395,7 @@ def run_ours(args):
     hbm_floor_ms = bytes_launch / (hbm_peak * 1e9) * 1e3
     alu_floor_ms = slots * samples_launch / alu_peak * 1e3
     hbm_roof = {"bound": "hbm", "achieved": bytes_launch / (k_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "traffic": None, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
+                "traffic": ncu_traffic(cfg.number), "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
                 "algorithmic_bytes_per_launch": bytes_launch, "floor_ms": hbm_floor_ms}
     hbm_roof["frac"] = hbm_roof["achieved"] / hbm_peak
     alu_roof = {"bound": "alu", "achieved": slots * samples_launch / (k_ms * 1e-3) / 1e12, "peak": alu_peak / 1e12,
@@ -364,13 +404,15 @@ def run_ours(args):
                 "algorithmic_slots_per_sample": slots, "floor_ms": alu_floor_ms}
     alu_roof["frac"] = alu_roof["achieved"] / alu_roof["peak"]
     primary, other = (alu_roof, hbm_roof) if alu_floor_ms > hbm_floor_ms else (hbm_roof, alu_roof)
-    primary = dict(primary, kernel="k_march (vr_render, single-march path)" if path == 1 else f"vr_render path {path}",
-                   kernel_ms=k_ms, launches_timed=len(render_ms))
+    kname = {1: "k_march_full (ray-major tiles)", 2: "k_march_bricks + k_composite (sort-last)",
+             7: "k_rows (lane-mapped rows; one or two launches per vr_render)"}.get(path, f"vr_render path {path}")
+    primary = dict(primary, kernel=kname, kernel_ms=k_ms, launches_timed=len(render_ms), zfast_copy=int(zfast))
 
     line = {"metric": "voxel_samples_per_s", "value": value, "unit": "samples/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": config_block(cfg), "clocks": clk,
+            "config": config_block(cfg, "" if len(view_ids) == cfg.n_views else f"ONLY views {view_ids} (profiling run)"),
+            "clocks": clk,
             "e2e": {"value": e2e_value, "unit": "samples/s", "h2d_bytes_per_step": int(h2d),
                     "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps},
             "gpu_launches": int(launches),
@@ -380,6 +422,8 @@ def run_ours(args):
                           "mean": k_ms, "max": float(np.max(render_ms))},
             "render_ms_by_view": [round(float(np.mean(render_ms[v::frames_step])), 4) for v in range(frames_step)],
             "render_share_of_step": float(np.sum(render_ms)) / ms_total,
+            "render_ms_cold": ({"mean": float(np.mean(cold_ms)), "max": float(np.max(cold_ms)),
+                                "note": "one orbit at unseen azimuths, outside the timed region"} if cold_ms else None),
             "effective_hbm_gbs_per_frame": 4.0 * n_vox / (k_ms * 1e-3) / 1e9,
             "samples_per_step": int(samples_step)}
     if world == 1 and not args.no_cpu:
@@ -576,13 +620,17 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (default 2 = configs[1])")
+    ap.add_argument("--config", type=int, default=4,
+                    help="BASELINE.json config number (default 4: the largest single-GPU config; the metric is 'per cube size')")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--ooc-nz", type=int, default=0, help="cfg5: spectral channels to use (0 = as many brick layers as fit host memory)")
     ap.add_argument("--ooc-resident-frac", type=float, default=0.25, help="cfg5: device brick pool as a fraction of the cube")
     ap.add_argument("--path", type=int, default=0, help="VR_OPT_RENDER_PATH for ablations (0 = auto, the product default)")
+    ap.add_argument("--lag", type=int, default=-1, help="VR_OPT_LANE_LAG for ablations (-1 = library default)")
+    ap.add_argument("--no-zcopy", action="store_true", help="VR_OPT_ZFAST_COPY = 0 (ablation)")
+    ap.add_argument("--views", type=int, default=0, help="render only the first N views of the orbit (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -77,7 +77,8 @@ typedef struct vr_volume vr_volume; /* opaque; created and destroyed only by the
  *                  queues (or streams) to overlap GPU computation with data I/O"): a pool of
  *                  floor(resident_bytes / brick_bytes) brick slots; bricks are streamed per
  *                  frame in view order on n_copy_streams streams.  Requires VR_BRICKED_HALO1.
- *   data       BORROWED until vr_destroy_volume; never written by the library.
+ *   data       BORROWED until vr_destroy_volume; never written by the library; its contents must
+ *              not change while the handle exists (the library may hold derived copies).
  *   n_copy_streams  1..8 (0 => 4).  Only used for VR_HOST_PINNED.
  * Errors: VR_ERR_INVALID_ARG (NULL, dims < 2, bad enums, brick grid too large, pageable host
  * memory, misaligned device pointer), VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA.
@@ -204,40 +205,35 @@ typedef struct {
     uint32_t n_bricks;              /* bricks in the grid */
     uint32_t bricks_drawn;          /* bricks that produced work in the last render */
     uint32_t bricks_culled;         /* bricks outside the view (empty screen rectangle) */
-    uint32_t path;                  /* last render: 0 none, 1 ray-major march, 2 sort-last, 3 brick chain, 4 tile-wave, 5 beam-slab (TMA boxes), 6 sheared-plane beams */
+    uint32_t path;                  /* last render: 0 none, 1 ray-major tiles, 2 sort-last, 3 brick chain, 7 lane-mapped rows */
     uint32_t kernel_launches;       /* library kernels launched by the last call */
     uint64_t fragments;             /* (brick,pixel) partial fragments written (sort-last) */
     uint64_t h2d_bytes;             /* host-to-device bytes enqueued by the last call */
     uint64_t d2h_bytes;             /* device-to-host bytes enqueued by the last call */
     uint64_t total_kernel_launches; /* since vr_create_volume */
     uint64_t resident_bytes;        /* device bytes owned by the handle */
-    uint32_t beam_overflow;         /* != 0: a beam-slab box exceeded its planned capacity (internal error; never expected) */
-    uint32_t beams_direct_total;    /* beams of the sheared-plane path marched from global memory because their planes
-                                       did not fit a shared-memory slot, since vr_create_volume (valid once the renders
-                                       have completed) */
+    uint32_t zfast_copy;            /* 1: the handle holds a z-fastest copy of the volume (VR_OPT_ZFAST_COPY) */
+    uint32_t reserved;
 } vr_stats;
 
 VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
 
 /* ------------------------------------------------------------------------------------------
- * vr_set_option — implementation choices that never change results beyond the documented
- * tolerances (all paths evaluate the same canonical arithmetic, C.1-C.7); used by the parity
- * tests to force each path and by bench.py for ablations.
- *   VR_OPT_RENDER_PATH  how a device-resident VR_LINEAR volume is marched when VR_SORT_LAST is
- *                       not requested: 0 = auto (sheared-plane beams when the camera is purely
- *                       perspective or purely orthographic and its beams fit shared memory, else
- *                       ray-major), 1 = ray-major (one thread per ray through global memory),
- *                       2 = tile-wave (shared-memory tiles in dataflow order; kept for ablation),
- *                       3 = beam-slab with TMA slab boxes (kept for ablation), 4 = sheared-plane
- *                       beams (3 and 4 fall back to ray-major like auto).
- *   VR_OPT_TILE_SHAPE   staging tile of the tile-wave path: 0 = auto, 1 = 32x32x32,
- *                       2 = 32x32x16, 3 = 32x16x16, 4 = 16x16x16 ownership cells.
- *   VR_OPT_SPARSE_DIRECT  experimental, default 0.  1: in the sheared-plane path, beams whose planes contain
- *                       x and whose rays would stage more than ~6 voxels per sample (sparse sampling: several
- *                       voxels per pixel) skip the staging and read through L1.  Same arithmetic, same results.
+ * vr_set_option — implementation choices that never change results (all paths evaluate the same
+ * canonical arithmetic, C.1-C.7, and are bit-identical); used by the parity tests and by bench.py.
+ *   VR_OPT_RENDER_PATH  how a resident VR_LINEAR volume is marched when VR_SORT_LAST is not requested:
+ *                       0 = auto: lane-mapped rows (one thread per ray; warps formed per frame so that their
+ *                       samples run along the memory-fast axis), 1 = ray-major (fixed 8x4-pixel warps).
+ *   VR_OPT_ZFAST_COPY   1 (default): the first view with rays that travel mostly along x makes the library
+ *                       allocate a z-fastest copy of a resident VR_LINEAR volume (same size as the volume,
+ *                       transposed once on the render's stream) when the device has that much free memory,
+ *                       and such rays are rendered from it; 0: never (they are rendered from the x-fastest
+ *                       array, slower).  The voxel data must not change while a handle holds a copy.
+ *   VR_OPT_LANE_LAG     lane-mapped path: a ray more than this many voxel planes (along the view's principal
+ *                       axis) ahead of the slowest ray of its warp waits; 0 = off; default 1.
  * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).
  * ------------------------------------------------------------------------------------------ */
-enum { VR_OPT_RENDER_PATH = 1, VR_OPT_TILE_SHAPE = 2, VR_OPT_SPARSE_DIRECT = 3 };
+enum { VR_OPT_RENDER_PATH = 1, VR_OPT_ZFAST_COPY = 2, VR_OPT_LANE_LAG = 3 };
 VR_API vr_status vr_set_option(vr_volume *vol, uint32_t option, int64_t value);
 
 /* Thread-local message of the last failing call on this thread ("" if none). */

@@ -18,8 +18,8 @@ VR_LINEAR, VR_BRICKED_HALO1 = 0, 1
 VR_DEVICE, VR_HOST_PINNED = 0, 1
 VR_EA, VR_MIP = 0, 1
 VR_SORT_LAST = 1
-VR_OPT_RENDER_PATH, VR_OPT_TILE_SHAPE, VR_OPT_SPARSE_DIRECT = 1, 2, 3
-VR_PATH_AUTO, VR_PATH_RAY_MAJOR, VR_PATH_TILE_WAVE, VR_PATH_BEAM_SLAB, VR_PATH_SHEAR = 0, 1, 2, 3, 4
+VR_OPT_RENDER_PATH, VR_OPT_ZFAST_COPY, VR_OPT_LANE_LAG = 1, 2, 3
+VR_PATH_AUTO, VR_PATH_RAY_MAJOR = 0, 1
 
 _STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_UNSUPPORTED", 3: "VR_ERR_OUT_OF_MEMORY",
            4: "VR_ERR_CUDA", 5: "VR_ERR_NOT_READY"}
@@ -54,7 +54,7 @@ class vr_stats(C.Structure):
                 ("bricks_culled", C.c_uint32), ("path", C.c_uint32), ("kernel_launches", C.c_uint32),
                 ("fragments", C.c_uint64), ("h2d_bytes", C.c_uint64), ("d2h_bytes", C.c_uint64),
                 ("total_kernel_launches", C.c_uint64), ("resident_bytes", C.c_uint64),
-                ("beam_overflow", C.c_uint32), ("beams_direct_total", C.c_uint32)]
+                ("zfast_copy", C.c_uint32), ("reserved", C.c_uint32)]
 
 
 EXPORTS = ("vr_create_volume", "vr_destroy_volume", "vr_set_transfer_function", "vr_render",
@@ -67,12 +67,9 @@ def library_path() -> str:
     return _build.LIB
 
 
-def load():
-    """dlopen libvr.so (building it with nvcc first if it is missing or stale)."""
-    global _lib
-    if _lib is None:
-        path = _build.build()
-        lib = C.CDLL(path)
+def _declare(lib):
+    """ctypes signatures of the entry points of include/vr.h."""
+    if True:
         lib.vr_create_volume.restype = C.c_int
         lib.vr_create_volume.argtypes = [C.POINTER(vr_volume_desc), C.POINTER(C.c_void_p)]
         lib.vr_destroy_volume.restype = C.c_int
@@ -89,7 +86,15 @@ def load():
         lib.vr_set_option.argtypes = [C.c_void_p, C.c_uint32, C.c_int64]
         lib.vr_last_error.restype = C.c_char_p
         lib.vr_version.restype = C.c_char_p
-        _lib = lib
+    return lib
+
+
+def load():
+    """dlopen libvr.so (building it with nvcc first if it is missing or stale).  There is nothing else to load:
+    no CPU implementation exists behind this binding."""
+    global _lib
+    if _lib is None:
+        _lib = _declare(C.CDLL(_build.build()))
     return _lib
 
 

@@ -99,15 +99,11 @@ struct vr_volume {
     vr_summary *d_sum_out = nullptr;          // staging for host outputs
     DevBuf<float> arena, host_image;
 
-    // tile-wave path
-    DevBuf<unsigned char> tile_work;
-    DevBuf<unsigned int> tile_ctrl, tile_done;
-    unsigned int tile_serial = 0;
-    uint64_t tile_done_sig = 0;               // tile grid the done flags were cleared for
-    int opt_path = 0, opt_tile = 0, opt_sparse = 0;   // vr_set_option
-    ShearPlanCache *shear_cache = nullptr;    // last per-frame plans of the sheared-plane path
-    unsigned int *beam_overflow_h = nullptr;  // mapped pinned words: [0] set if a staged box / plane overflowed, [1] beams marched from global memory
-    unsigned int *beam_overflow_d = nullptr;
+    // lane-mapped path: the library's z-fastest copy of a resident linear volume (vr_lanes.cu)
+    float *zfast = nullptr;
+    bool zfast_failed = false;                // allocation refused once: not retried
+    cudaEvent_t zfast_ev = nullptr;           // recorded after the transposition
+    int opt_path = 0, opt_zcopy = 1, opt_lag = 1;   // vr_set_option
     Staging staging[kStagingRing];
     int staging_next = 0;
 
@@ -134,11 +130,10 @@ static void free_volume(vr_volume *v)
     if (v->d_tf) cudaFree(v->d_tf);
     if (v->d_sum) cudaFree(v->d_sum);
     if (v->d_sum_out) cudaFree(v->d_sum_out);
-    if (v->beam_overflow_h) cudaFreeHost(v->beam_overflow_h);
-    shear_cache_destroy(v->shear_cache);
+    if (v->zfast) cudaFree(v->zfast);
+    if (v->zfast_ev) cudaEventDestroy(v->zfast_ev);
     v->arena.release();
     v->host_image.release();
-    v->tile_work.release(); v->tile_ctrl.release(); v->tile_done.release();
     delete v;
 }
 
@@ -411,124 +406,70 @@ static vr_status render_chain(vr_volume *v, const vr_camera *c, const CamK &cam,
     return VR_OK;
 }
 
-// tile-wave march of a device-resident linear volume (vr_tiles.cu): exact ERT, one pass over the voxels
-static bool tiles_applicable(const vr_volume *v, const vr_camera *c, bool persp, bool ortho)
+// ------------------------------------------------------------------ lane-mapped single march (vr_lanes.cu)
+// The z-fastest copy is made lazily, the first time a view has pixels that travel mostly along x, when
+// the option allows it and the device has room; without it such pixels are rendered from the x-fastest
+// array (same results, slower).
+static vr_status ensure_zfast(vr_volume *v, cudaStream_t st, bool *have)
 {
-    if (v->opt_path != 2) return false;                       // tile-wave only on request (ablation)
-    if (v->desc.layout != VR_LINEAR || v->out_of_core || !(persp || ortho)) return false;
-    (void)c;
-    return true;
+    *have = false;
+    if (!v->opt_zcopy || v->desc.layout != VR_LINEAR || v->out_of_core || v->zfast_failed) return VR_OK;
+    if (!v->zfast) {
+        const size_t bytes = (size_t)v->n_vox * sizeof(float);
+        size_t free_b = 0, total_b = 0;
+        VR_CUDA(cudaMemGetInfo(&free_b, &total_b));
+        if ((v->desc.nz + 31) / 32 > 65535u || free_b < bytes + ((size_t)512 << 20)) { v->zfast_failed = true; return VR_OK; }
+        float *p = nullptr;
+        if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); v->zfast_failed = true; return VR_OK; }
+        v->zfast = p;
+        if (!v->zfast_ev) VR_CUDA(cudaEventCreateWithFlags(&v->zfast_ev, cudaEventDisableTiming));
+        launch_transpose_xz(v->dev_data, v->zfast, (int)v->desc.nx, (int)v->desc.ny, (int)v->desc.nz, st);
+        VR_CUDA(cudaEventRecord(v->zfast_ev, st));
+        v->stats.kernel_launches += (v->desc.ny + 65534) / 65535;
+        v->stats.resident_bytes += bytes;
+    }
+    VR_CUDA(cudaStreamWaitEvent(st, v->zfast_ev, 0));
+    *have = true;
+    return VR_OK;
 }
 
-static vr_status render_tiles(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, bool persp,
-                              const TfK &tf, float *img, long long pitch_f, cudaStream_t st)
+static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, const TfK &tf,
+                              float *img, long long pitch_f, cudaStream_t st)
 {
     const int n[3] = { (int)v->desc.nx, (int)v->desc.ny, (int)v->desc.nz };
-    int kind = v->opt_tile;
-    if (kind <= 0 || kind >= VR_TILE_KINDS) kind = VR_TILE_32x32x16;
-    TilePlanK P;
-    tile_dims(kind, P.T);
-    P.persp = persp ? 1 : 0;
-    long long n_tiles = 1;
-    int max_lvl[3];
-    for (int a = 0; a < 3; ++a) {
-        P.nt[a] = std::max(1, (n[a] - 1 + P.T[a] - 1) / P.T[a]);       // base indices 0 .. n-2
-        n_tiles *= P.nt[a];
-        const float oc = c->o0[a] - 0.5f;                              // float32, as make_ray forms it (C.3)
-        const double fl = std::floor((double)oc);
-        const long long fi = (long long)std::min(std::max(fl, -1e15), 1e15);
-        long long e = fi >= 0 ? fi / P.T[a] : -((-fi + P.T[a] - 1) / P.T[a]);
-        e = std::min<long long>(std::max<long long>(e, -(1 << 28)), 1 << 28);
-        P.e[a] = (int)e;
-        P.sgn[a] = c->d0[a] > 0.0f ? 1 : c->d0[a] < 0.0f ? -1 : 0;
-        P.lvl0[a] = 0;
-        if (persp) {
-            P.lvl0[a] = P.e[a] < 0 ? -P.e[a] : P.e[a] > P.nt[a] - 1 ? P.e[a] - (P.nt[a] - 1) : 0;
-            max_lvl[a] = std::max(tile_axis_level(P, a, 0), tile_axis_level(P, a, P.nt[a] - 1));
-        } else max_lvl[a] = P.sgn[a] ? P.nt[a] - 1 : 0;
+    // how many of 9 probe pixels (corners, edge midpoints, centre) travel mostly along x
+    int n_x = 0;
+    for (int py = 0; py < 3; ++py)
+        for (int px = 0; px < 3; ++px) {
+            const double x = 0.5 * px * cam.width, y = 0.5 * py * cam.height;
+            const double gx = (double)c->d0[0] + x * (double)c->du[0] + y * (double)c->dv[0];
+            const double gz = (double)c->d0[2] + x * (double)c->du[2] + y * (double)c->dv[2];
+            if (std::fabs(gx) > std::fabs(gz)) ++n_x;
+        }
+    bool have_z = false;
+    if (n_x > 0) { vr_status rc = ensure_zfast(v, st, &have_z); if (rc != VR_OK) return rc; }
+    LaneVolK A, Z;
+    A.base = v->dev_data; A.sa = n[0]; A.sb = (long long)n[0] * n[1]; A.nx = n[0]; A.ny = n[1]; A.nz = n[2];
+    Z = A; Z.base = v->zfast; Z.sa = (long long)n[1] * n[2]; Z.sb = n[2];
+    LaneMapK M;
+    int rows;
+    if (!have_z || n_x == 0) {
+        make_lane_map(c, n, 0, 0, v->opt_lag, M, rows);
+        launch_rows(mode, ert, cam, A, 0, tf, M, rows, img, pitch_f, st);
+        v->stats.kernel_launches += 1;
+    } else if (n_x == 9) {
+        make_lane_map(c, n, 2, 0, v->opt_lag, M, rows);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, rows, img, pitch_f, st);
+        v->stats.kernel_launches += 1;
+    } else {
+        make_lane_map(c, n, 0, 1, v->opt_lag, M, rows);
+        launch_rows(mode, ert, cam, A, 0, tf, M, rows, img, pitch_f, st);
+        make_lane_map(c, n, 2, 2, v->opt_lag, M, rows);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, rows, img, pitch_f, st);
+        v->stats.kernel_launches += 2;
     }
-    if (n_tiles > 0x3fffffffll || P.nt[0] > 65535 || P.nt[1] > 65535 || P.nt[2] > 65535) {
-        set_error("tile grid too large"); return VR_ERR_UNSUPPORTED;
-    }
-    P.n_tiles = (int)n_tiles;
-    P.n_levels = max_lvl[0] + max_lvl[1] + max_lvl[2] + 1;
-
-    // tiles per level = convolution of the three per-axis level histograms
-    std::vector<unsigned long long> hx(max_lvl[0] + 1, 0), hy(max_lvl[1] + 1, 0), hz(max_lvl[2] + 1, 0), hxy(max_lvl[0] + max_lvl[1] + 1, 0);
-    for (int b = 0; b < P.nt[0]; ++b) hx[tile_axis_level(P, 0, b)]++;
-    for (int b = 0; b < P.nt[1]; ++b) hy[tile_axis_level(P, 1, b)]++;
-    for (int b = 0; b < P.nt[2]; ++b) hz[tile_axis_level(P, 2, b)]++;
-    for (size_t i = 0; i < hx.size(); ++i) for (size_t j = 0; j < hy.size(); ++j) hxy[i + j] += hx[i] * hy[j];
-    std::vector<unsigned long long> cnt(P.n_levels, 0);
-    for (size_t i = 0; i < hxy.size(); ++i) if (hxy[i]) for (size_t j = 0; j < hz.size(); ++j) cnt[i + j] += hxy[i] * hz[j];
-
-    Staging *s;
-    vr_status rc = staging_acquire(v, (size_t)(P.n_levels + 1) * sizeof(unsigned int), &s);
-    if (rc != VR_OK) return rc;
-    unsigned int *off = reinterpret_cast<unsigned int *>(s->h);
-    unsigned long long acc = 0;
-    for (int l = 0; l < P.n_levels; ++l) { off[l] = (unsigned int)acc; acc += cnt[l]; }
-    off[P.n_levels] = (unsigned int)acc;
-    if (acc != (unsigned long long)n_tiles) { set_error("internal: tile level counts do not add up"); return VR_ERR_UNSUPPORTED; }
-
-    if ((rc = v->tile_work.reserve((size_t)n_tiles * sizeof(TileWork))) != VR_OK) return rc;
-    if ((rc = v->tile_ctrl.reserve((size_t)P.n_levels + 1)) != VR_OK) return rc;
-    const uint64_t sig = ((uint64_t)kind << 32) | (uint64_t)n_tiles;
-    if (v->tile_done.cap < (size_t)n_tiles || sig != v->tile_done_sig) {
-        if ((rc = v->tile_done.reserve((size_t)n_tiles)) != VR_OK) return rc;
-        VR_CUDA(cudaMemsetAsync(v->tile_done.p, 0, v->tile_done.cap * sizeof(unsigned int), st));
-        v->tile_done_sig = sig;
-    }
-    const unsigned int serial = ++v->tile_serial;
-
-    VolK V;
-    V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
-    V.nx = n[0]; V.ny = n[1]; V.nz = n[2]; V.ox = V.oy = V.oz = 0;
-    VR_CUDA(cudaMemsetAsync(v->tile_ctrl.p, 0, ((size_t)P.n_levels + 1) * sizeof(unsigned int), st));
-    VR_CUDA(cudaMemcpyAsync(s->d, s->h, (size_t)(P.n_levels + 1) * sizeof(unsigned int), cudaMemcpyHostToDevice, st));
-    v->stats.h2d_bytes += (size_t)(P.n_levels + 1) * sizeof(unsigned int);
-    launch_tile_plan(cam, P, V, reinterpret_cast<const unsigned int *>(s->d), v->tile_ctrl.p,
-                     reinterpret_cast<TileWork *>(v->tile_work.p), st);
-    launch_chain_init(mode, cam.width, cam.height, img, pitch_f, st);
-    rc = launch_tile_march(kind, mode, ert, cam, P, V, tf, reinterpret_cast<const TileWork *>(v->tile_work.p),
-                           v->tile_ctrl.p, v->tile_done.p, serial, img, pitch_f, v->sm_count, st);
-    if (rc != VR_OK) return rc;
-    v->stats.kernel_launches += 3;
-    if (mode == VR_EA) { launch_chain_finish(cam.width, cam.height, img, pitch_f, st); v->stats.kernel_launches += 1; }
-    VR_CUDA(cudaEventRecord(s->done, st));
-    s->in_flight = true;
-    v->stats.path = 4;
-    v->stats.bricks_drawn = (uint32_t)n_tiles;
-    return VR_OK;
-}
-
-
-// beam-slab march of a device-resident linear volume (vr_beam.cu): one launch, exact ERT, ray state in registers
-static vr_status render_beam(vr_volume *v, const CamK &cam, int mode, bool ert, const TfK &tf, float *img,
-                             long long pitch_f, cudaStream_t st, bool *applied)
-{
-    VolK V;
-    V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
-    V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz; V.ox = V.oy = V.oz = 0;
-    vr_status rc = launch_beam(mode, ert, cam, V, tf, v->beam_overflow_d, img, pitch_f, st, applied);
-    if (rc != VR_OK || !*applied) return rc;
-    v->stats.kernel_launches += 1;
-    v->stats.path = 5;
-    v->stats.bricks_drawn = (uint32_t)v->n_bricks;
-    return VR_OK;
-}
-
-// sheared-plane beam march of a device-resident linear volume (vr_shear.cu): one launch, exact ERT
-static vr_status render_shear(vr_volume *v, const CamK &cam, int mode, bool ert, const TfK &tf, float *img,
-                              long long pitch_f, cudaStream_t st, bool *applied)
-{
-    VolK V;
-    V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
-    V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz; V.ox = V.oy = V.oz = 0;
-    vr_status rc = launch_shear(mode, ert, v->opt_sparse != 0, cam, V, tf, v->beam_overflow_d, v->shear_cache, img, pitch_f, st, applied);
-    if (rc != VR_OK || !*applied) return rc;
-    v->stats.kernel_launches += 1;
-    v->stats.path = 6;
+    v->stats.path = 7;
+    v->stats.zfast_copy = v->zfast ? 1u : 0u;
     v->stats.bricks_drawn = (uint32_t)v->n_bricks;
     return VR_OK;
 }
@@ -623,10 +564,6 @@ VR_API vr_status vr_create_volume(const vr_volume_desc *d, vr_volume **out)
     VR_FAIL_CUDA(cudaMalloc(&v->d_tf, 257 * sizeof(float4)));
     VR_FAIL_CUDA(cudaMalloc(&v->d_sum, sizeof(SummaryScratch)));
     VR_FAIL_CUDA(cudaMalloc(&v->d_sum_out, VR_SUMMARY_BYTES(4096)));
-    VR_FAIL_CUDA(cudaHostAlloc(&v->beam_overflow_h, 2 * sizeof(unsigned int), cudaHostAllocMapped));
-    v->beam_overflow_h[0] = v->beam_overflow_h[1] = 0u;
-    VR_FAIL_CUDA(cudaHostGetDevicePointer(&v->beam_overflow_d, v->beam_overflow_h, 0));
-    v->shear_cache = shear_cache_create();       // nullptr (allocation failure) only means no caching
 #undef VR_FAIL_CUDA
     *out = v;
     return VR_OK;
@@ -710,15 +647,8 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     TfK tf; tf.table = v->d_tf; tf.scale = v->tf_scale; tf.bias = v->tf_bias;
     if (sort_last) rc = render_sort_last(v, c, cam, mode, tf, img, pitch_f, st);
     else if (v->out_of_core || v->desc.layout == VR_BRICKED_HALO1) rc = render_chain(v, c, cam, mode, ert, tf, img, pitch_f, st);
-    else if (tiles_applicable(v, c, persp, ortho)) rc = render_tiles(v, c, cam, mode, ert, persp, tf, img, pitch_f, st);
-    else {
-        bool applied = false;
-        if ((v->opt_path == 0 || v->opt_path == 4) && (persp || ortho))
-            rc = render_shear(v, cam, mode, ert, tf, img, pitch_f, st, &applied);
-        if (rc == VR_OK && !applied && v->opt_path == 3 && (persp || ortho))
-            rc = render_beam(v, cam, mode, ert, tf, img, pitch_f, st, &applied);
-        if (rc == VR_OK && !applied) rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
-    }
+    else if (v->opt_path == 1) rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
+    else rc = render_lanes(v, c, cam, mode, ert, tf, img, pitch_f, st);
     if (rc != VR_OK) return rc;
     VR_CUDA(cudaGetLastError());
     if (im->location == VR_HOST_PINNED) {
@@ -808,14 +738,14 @@ VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
     VR_REQUIRE(v, "vr_set_option: NULL handle");
     switch (option) {
     case VR_OPT_RENDER_PATH:
-        VR_REQUIRE(value >= 0 && value <= 4, "VR_OPT_RENDER_PATH: 0 auto, 1 ray-major, 2 tile-wave, 3 beam-slab (TMA), 4 sheared planes (got %lld)", (long long)value);
+        VR_REQUIRE(value == 0 || value == 1, "VR_OPT_RENDER_PATH: 0 auto (lane-mapped), 1 ray-major tiles (got %lld)", (long long)value);
         v->opt_path = (int)value; return VR_OK;
-    case VR_OPT_TILE_SHAPE:
-        VR_REQUIRE(value >= 0 && value < VR_TILE_KINDS, "VR_OPT_TILE_SHAPE: 0..%d (got %lld)", VR_TILE_KINDS - 1, (long long)value);
-        v->opt_tile = (int)value; return VR_OK;
-    case VR_OPT_SPARSE_DIRECT:
-        VR_REQUIRE(value == 0 || value == 1, "VR_OPT_SPARSE_DIRECT: 0 or 1 (got %lld)", (long long)value);
-        v->opt_sparse = (int)value; return VR_OK;
+    case VR_OPT_ZFAST_COPY:
+        VR_REQUIRE(value == 0 || value == 1, "VR_OPT_ZFAST_COPY: 0 never, 1 when needed and it fits (got %lld)", (long long)value);
+        v->opt_zcopy = (int)value; return VR_OK;
+    case VR_OPT_LANE_LAG:
+        VR_REQUIRE(value >= 0 && value <= 1024, "VR_OPT_LANE_LAG: 0..1024 base planes (got %lld)", (long long)value);
+        v->opt_lag = (int)value; return VR_OK;
     default:
         set_error("unknown option %u", option); return VR_ERR_INVALID_ARG;
     }
@@ -827,8 +757,6 @@ VR_API vr_status vr_get_stats(vr_volume *v, vr_stats *s)
     VR_REQUIRE(v && s, "vr_get_stats: NULL argument");
     VR_REQUIRE(s->struct_size == sizeof(vr_stats), "vr_stats.struct_size %u != %zu", s->struct_size, sizeof(vr_stats));
     *s = v->stats;
-    s->beam_overflow = v->beam_overflow_h ? reinterpret_cast<volatile unsigned int *>(v->beam_overflow_h)[0] : 0u;
-    s->beams_direct_total = v->beam_overflow_h ? reinterpret_cast<volatile unsigned int *>(v->beam_overflow_h)[1] : 0u;
     return VR_OK;
 }
 

@@ -1,11 +1,14 @@
 // vr_internal.h — host-side handle, error plumbing and kernel launcher declarations.
 #pragma once
+#ifndef VR_SIMT_HOST               // tests/simt/simt_host.h (force-included by the host emulation build) stands in
 #include <cuda_runtime.h>
+#endif
 #include <stdint.h>
 #include <string>
 #include <vector>
 
 #include "../../include/vr.h"
+#include "vr_lanemap.h"
 #include "vr_math.cuh"
 
 namespace vr {
@@ -23,6 +26,26 @@ vr_status cuda_fail(cudaError_t e, const char *what);
     do {                                                               \
         if (!(cond)) { ::vr::set_error(__VA_ARGS__); return VR_ERR_INVALID_ARG; } \
     } while (0)
+
+// Every kernel launch of the library goes through here (one place for the launch syntax; the host emulation
+// build of the tests runs the same kernel function thread by thread instead).
+template <typename... P, typename... A>
+inline void vr_launch(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, A &&...args)
+{
+#ifdef VR_SIMT_HOST
+    (void)st;
+    ::simt::launch(grid, block, smem, [&] { kernel(static_cast<P>(args)...); });
+#else
+    kernel<<<grid, block, smem, st>>>(static_cast<P>(args)...);
+#endif
+}
+
+// dynamic shared memory of the CTA as an array of T
+#ifdef VR_SIMT_HOST
+#define VR_DYN_SHARED(T, name) T *name = reinterpret_cast<T *>(::simt::g_dyn_smem)
+#else
+#define VR_DYN_SHARED(T, name) extern __shared__ T name[]
+#endif
 
 // ---------------------------------------------------------------- reductions (vr_reduce.cu)
 // device scratch of one summary call
@@ -81,68 +104,18 @@ void launch_chain_brick(int mode, bool ert, const CamK &cam, const VolK &vol, co
                         float *image, long long pitch_f, cudaStream_t st);
 void launch_chain_finish(int W, int H, float *image, long long pitch_f, cudaStream_t st);
 
-// ---------------------------------------------------------------- tile-wave ray casting (vr_tiles.cu)
-// The volume is cut into staging tiles of TX x TY x TZ ownership cells (a finer brick grid, C.7).
-// A persistent kernel stages one tile at a time in shared memory and marches every ray segment
-// that crosses it; tiles are taken front to back (level = per-axis tile distance from the eye
-// tile) and a tile starts once its <= 3 face neighbours towards the eye are complete, so the ray
-// state carried in the image sees its samples in k order (exact C.5 / ERT).
-struct TileWork {                // one entry of the per-frame work list (level-major)
-    int x0, y0, x1, y1;          // conservative screen rectangle, [x0,x1) x [y0,y1); empty => no work
-    unsigned short b[3];         // tile coordinates
-    unsigned short flags;
+// ---------------------------------------------------------------- lane-mapped ray casting (vr_lanes.cu)
+// A resident volume as the kernel addresses it: one axis has element stride 1 (`fast`: 0 = the caller's
+// x-fastest array, 2 = the library's z-fastest copy); sa, sb are the element strides of the other two
+// axes in ascending axis order (fast 0: y, z; fast 2: x, y).
+struct LaneVolK {
+    const float *base;
+    long long sa, sb;
+    int nx, ny, nz;
 };
 
-struct TilePlanK {
-    int nt[3];                   // tiles per axis
-    int T[3];                    // tile edge per axis
-    int persp;                   // 1: pure perspective (ou = ov = 0); 0: pure orthographic (du = dv = 0)
-    int e[3];                    // perspective: tile index of the eye, floor(floor(o0 - 0.5) / T), unclamped
-    int sgn[3];                  // orthographic: sign of d0 per axis
-    int lvl0[3];                 // per-axis minimum raw level (subtracted so that levels start at 0)
-    int n_tiles, n_levels;
-};
-
-__host__ __device__ inline int tile_axis_level(const TilePlanK &P, int a, int b)
-{
-    if (P.persp) return (b > P.e[a] ? b - P.e[a] : P.e[a] - b) - P.lvl0[a];
-    return P.sgn[a] > 0 ? b : P.sgn[a] < 0 ? P.nt[a] - 1 - b : 0;
-}
-// tile coordinate of the face neighbour towards the eye on axis a, or -1
-__host__ __device__ inline int tile_axis_pred(const TilePlanK &P, int a, int b)
-{
-    int p;
-    if (P.persp) p = b > P.e[a] ? b - 1 : b < P.e[a] ? b + 1 : -1;
-    else p = P.sgn[a] > 0 ? b - 1 : P.sgn[a] < 0 ? b + 1 : -1;
-    return (p < 0 || p >= P.nt[a]) ? -1 : p;
-}
-
-enum { VR_TILE_32 = 1, VR_TILE_32x32x16 = 2, VR_TILE_32x16x16 = 3, VR_TILE_16 = 4, VR_TILE_KINDS = 5 };
-void tile_dims(int kind, int T[3]);
-// ctrl: [0] pop counter, [1 .. n_levels] per-level fill cursors (zeroed before each frame)
-void launch_tile_plan(const CamK &cam, const TilePlanK &P, const VolK &vol, const unsigned int *lvl_off,
-                      unsigned int *ctrl, TileWork *work, cudaStream_t st);
-vr_status launch_tile_march(int kind, int mode, bool ert, const CamK &cam, const TilePlanK &P, const VolK &vol,
-                            const TfK &tf, const TileWork *work, unsigned int *ctrl, unsigned int *done,
-                            unsigned int serial, float *image, long long pitch_f, int sm_count, cudaStream_t st);
-
-
-// ---------------------------------------------------------------- beam-slab ray casting (vr_beam.cu)
-// One CTA per 16x16-pixel beam, ray state in registers, the beam's voxel box staged slab by slab in
-// shared memory by TMA (double buffered).  *applied = false: camera / volume outside what the path
-// handles (very wide beams, boxes larger than shared memory) — nothing was enqueued.
-vr_status launch_beam(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, unsigned int *overflow_dev,
-                      float *image, long long pitch_f, cudaStream_t st, bool *applied);
-
-
-// ---------------------------------------------------------------- sheared-plane beam ray casting (vr_shear.cu)
-// Same beams, but every data plane of a slab is staged as its own rectangle at its own origin by 4-byte
-// cp.async into a bank-conflict-aware layout.  *applied = false: nothing was enqueued.
-struct ShearPlanCache;                       // per-handle cache of the per-frame host plans (camera -> plan)
-ShearPlanCache *shear_cache_create();
-void shear_cache_destroy(ShearPlanCache *c);
-vr_status launch_shear(int mode, bool ert, bool sparse_direct, const CamK &cam, const VolK &vol, const TfK &tf,
-                       unsigned int *overflow_dev, ShearPlanCache *cache, float *image, long long pitch_f,
-                       cudaStream_t st, bool *applied);
+void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
+                 int rows, float *image, long long pitch_f, cudaStream_t st);
+void launch_transpose_xz(const float *in, float *out, int nx, int ny, int nz, cudaStream_t st);
 
 }  // namespace vr

@@ -1,0 +1,198 @@
+// vr_lanes.cu — the default ray-caster of resident linear volumes: one thread per ray, ray state in
+// registers from the first sample to the last (exact C.5 / ERT), the 8 corner voxels of every sample read
+// straight from global memory through L1 ("the GPU part").
+//
+// What decides the speed of such a kernel on B200 is the number of distinct 128-byte lines the 32 lanes of
+// a warp touch per corner load: the L1 pipe retires about one line per clock per SM, and the path issues 8
+// loads per sample.  The design therefore chooses, per frame, WHICH 32 rays form a warp so that their
+// samples at equal k run along the memory-fast axis of the volume:
+//   * lanes run along the image axis (u or v) whose footprint on the principal plane of the view moves
+//     most along the fast axis, and the image rows are SHEARED by an integer row offset off(p) =
+//     floor(sigma p + 1/2) of the lane coordinate p, so that a warp follows one row of voxels instead of
+//     drifting across rows (any function off(p) gives a bijection of the pixels: sigma only affects speed);
+//   * the sample lattice of C.2 is anchored at the volume entry, so the lanes of a warp start on the same
+//     entry face; a lane that gets more than `lag` base planes ahead of the slowest active lane of its warp
+//     waits one iteration, which keeps the 32 samples of an iteration on one or two data planes;
+//   * rays that travel mostly along x cannot be served from an x-fastest array (every lane would sit on its
+//     own line): the library keeps a second, z-fastest copy of the volume (vr_api.cu, made once, lazily)
+//     and such pixels are rendered from it by the same kernel with permuted strides.  A pixel belongs to
+//     the x-fastest copy iff |d_x| <= |d_z|.
+// All arithmetic is the canonical sequence of vr_math.cuh; indices are the clamped base indices of C.3, so
+// every address formed here is inside the volume by construction.
+#include <climits>
+
+#include "vr_internal.h"
+
+namespace vr {
+
+namespace {
+
+constexpr int kRowsPerCta = 8, kLaneThreads = 32 * kRowsPerCta;
+
+// transfer function in shared memory as two float2 tables ((r,g) and (b,a)); entry 256 = copy of 255
+struct TfS { float2 rg[257], ba[257]; };
+
+__device__ __forceinline__ void stage_tf_pairs(TfS &s, const TfK &tf)
+{
+    for (int e = threadIdx.x; e < 257; e += kLaneThreads) {
+        const float4 v = __ldg(tf.table + e);
+        s.rg[e] = make_float2(v.x, v.y);
+        s.ba[e] = make_float2(v.z, v.w);
+    }
+    __syncthreads();
+}
+
+// C.4 with the four channel lerps paired (same operations and operands as classify() of vr_math.cuh)
+__device__ __forceinline__ float4 classify_s(const TfS &s, float scale, float bias, float v)
+{
+    const float u = __saturatef(__fmaf_rn(v, scale, bias));
+    const float x = __fmul_rn(u, 255.0f);
+    const int i = min(__float2int_rz(x), 254);
+    const float f = __fsub_rn(x, (float)i);
+    const float2 rg = lerp_ee2(s.rg[i], s.rg[i + 1], f);
+    const float2 ba = lerp_ee2(s.ba[i], s.ba[i + 1], f);
+    return make_float4(rg.x, rg.y, ba.x, ba.y);
+}
+
+// C.5 with the r and g accumulations paired
+__device__ __forceinline__ void composite_p(float4 rgba, float &Cr, float &Cg, float &Cb, float &T)
+{
+    const float w = __fmul_rn(T, rgba.w);
+    const float2 c = fma2_rn(make_float2(w, w), make_float2(rgba.x, rgba.y), make_float2(Cr, Cg));
+    Cr = c.x; Cg = c.y;
+    Cb = __fmaf_rn(w, rgba.z, Cb);
+    T = __fsub_rn(T, w);
+}
+
+// the 8 corners of base index (ix,iy,iz): FAST = the axis with element stride 1 (0: x-fastest array,
+// 2: z-fastest copy); sa, sb = element strides of the other two axes in ascending axis order
+template <bool WIDE, int FAST>
+__device__ __forceinline__ float sample_cell(const LaneVolK &V, int ix, int iy, int iz, float fx, float fy, float fz)
+{
+    const int ia = FAST == 0 ? iy : ix, ib = FAST == 0 ? iz : iy, iu = FAST == 0 ? ix : iz;
+    const float *p;
+    if (WIDE) p = V.base + ((long long)ib * V.sb + (long long)ia * V.sa + iu);
+    else p = V.base + ((unsigned int)ib * (unsigned int)V.sb + (unsigned int)ia * (unsigned int)V.sa + (unsigned int)iu);
+    const float *pa = p + V.sa, *pb = p + V.sb, *pab = pb + V.sa;
+    const float q00 = __ldg(p), q01 = __ldg(p + 1);          // (a, b) = (0, 0): unit-stride neighbours
+    const float q10 = __ldg(pa), q11 = __ldg(pa + 1);        // a + 1
+    const float r00 = __ldg(pb), r01 = __ldg(pb + 1);        // b + 1
+    const float r10 = __ldg(pab), r11 = __ldg(pab + 1);      // a + 1, b + 1
+    // trilerp_packed(v000, v100, v010, v110, v001, v101, v011, v111): corner (X,Y,Z)
+    if (FAST == 0)      // u = x, a = y, b = z
+        return trilerp_packed(q00, q01, q10, q11, r00, r01, r10, r11, fx, fy, fz);
+    else                // u = z, a = x, b = y
+        return trilerp_packed(q00, q10, r00, r10, q01, q11, r01, r11, fx, fy, fz);
+}
+
+template <int MODE, bool ERT, bool WIDE, int FAST>
+__global__ void __launch_bounds__(kLaneThreads)
+k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, float *__restrict__ image, long long pitch_f)
+{
+    __shared__ TfS tf_s;
+    if (MODE == VR_EA) stage_tf_pairs(tf_s, tf);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // pixel of this lane: p along the lane axis, q = sheared row + off(p)
+    const int p = blockIdx.x * 32 + lane;
+    const int q = M.q_lo + (int)blockIdx.y * kRowsPerCta + warp + __float2int_rd(__fmaf_rn(M.sigma, (float)p, 0.5f));
+    const int i = M.lane_axis == 0 ? p : q, j = M.lane_axis == 0 ? q : p;
+    const bool inside = i >= 0 && i < cam.width && j >= 0 && j < cam.height;
+    Ray r;
+    bool mine = false, alive = false;
+    if (inside) {
+        const bool hit = make_ray(cam, V.nx, V.ny, V.nz, i, j, r);
+        const bool xmajor = fabsf(r.d[0]) > fabsf(r.d[2]);
+        mine = M.cls == 0 || (M.cls == 2) == xmajor;
+        // a direction that is not finite (d0 + px du + py dv = 0) has no defined samples: treated as a miss
+        alive = mine && hit && r.t_exit < CUDART_INF_F;
+    }
+    if (!__any_sync(0xffffffffu, mine)) return;
+    if (!alive) { r.t_first = 0.0f; r.t_exit = 0.0f; r.d[0] = r.d[1] = r.d[2] = 0.0f; r.oc[0] = r.oc[1] = r.oc[2] = 0.0f; }
+    float cr = 0.0f, cg = 0.0f, cb = 0.0f, T = 1.0f, m = -CUDART_INF_F;
+    float kf = 0.0f;
+    const int lag = M.lag;
+    for (;;) {
+        const float t = __fmaf_rn(kf, cam.step, r.t_first);
+        alive = alive && t < r.t_exit;                               // C.2: sample k exists iff t_k < t_exit
+        if (!__any_sync(0xffffffffu, alive)) break;
+        int ix, iy, iz;
+        float fx, fy, fz;
+        axis_cell(t, r.d[0], r.oc[0], V.nx, ix, fx);
+        axis_cell(t, r.d[1], r.oc[1], V.ny, iy, fy);
+        axis_cell(t, r.d[2], r.oc[2], V.nz, iz, fz);
+        bool go = alive;
+        if (lag > 0) {
+            const int ip = M.paxis == 0 ? ix : M.paxis == 1 ? iy : iz;
+            const int prog = M.psign >= 0 ? ip : -ip;
+            const int slowest = __reduce_min_sync(0xffffffffu, alive ? prog : INT_MAX);
+            go = alive && prog - slowest <= lag;
+        }
+        if (go) {
+            const float s = sample_cell<WIDE, FAST>(V, ix, iy, iz, fx, fy, fz);
+            if (MODE == VR_MIP) m = fmaxf(m, s);
+            else {
+                composite_p(classify_s(tf_s, tf.scale, tf.bias, s), cr, cg, cb, T);
+                if (ERT && T <= cam.t_min) alive = false;           // stop AFTER compositing this sample (C.5)
+            }
+            kf = __fadd_rn(kf, 1.0f);                                // exact: k < 2^24
+        }
+    }
+    if (!mine) return;
+    if (MODE == VR_MIP) image[(long long)j * pitch_f + i] = m;
+    else
+        *reinterpret_cast<float4 *>(image + (long long)j * pitch_f + 4 * (long long)i) =
+            make_float4(cr, cg, cb, __fsub_rn(1.0f, T));
+}
+
+// z-fastest copy: out[x][y][z] = in[z][y][x]; one CTA transposes a 32 (x) by 32 (z) tile of one y
+__global__ void __launch_bounds__(256)
+k_transpose_xz(const float *__restrict__ in, float *__restrict__ out, int nx, int ny, int nz)
+{
+    __shared__ float tile[32][33];
+    const int y = blockIdx.z, x0 = blockIdx.x * 32, z0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int r = ty; r < 32; r += 8) {
+        const int x = x0 + tx, z = z0 + r;
+        if (x < nx && z < nz) tile[r][tx] = __ldg(in + ((long long)z * ny + y) * nx + x);
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const int x = x0 + r, z = z0 + tx;
+        if (x < nx && z < nz) out[((long long)x * ny + y) * nz + z] = tile[tx][r];
+    }
+}
+
+}  // namespace
+
+void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
+                 int rows, float *image, long long pitch_f, cudaStream_t st)
+{
+    const int P = map.lane_axis == 0 ? cam.width : cam.height;
+    const dim3 g((unsigned)((P + 31) / 32), (unsigned)((rows + kRowsPerCta - 1) / kRowsPerCta));
+    if (g.x == 0 || g.y == 0) return;
+    const unsigned long long span = (unsigned long long)((fast == 0 ? vol.nz : vol.ny) - 1) * (unsigned long long)vol.sb +
+                                    (unsigned long long)((fast == 0 ? vol.ny : vol.nx) - 1) * (unsigned long long)vol.sa +
+                                    (unsigned long long)(fast == 0 ? vol.nx : vol.nz);
+    const bool wide = span > 0xffffffffull;
+#define VR_L3(M, E, Wd, F) vr_launch(k_rows<M, E, Wd, F>, g, kLaneThreads, 0, st, cam, vol, tf, map, image, pitch_f)
+#define VR_L2(M, E, Wd) do { if (fast == 0) VR_L3(M, E, Wd, 0); else VR_L3(M, E, Wd, 2); } while (0)
+#define VR_L1(M, E) do { if (wide) VR_L2(M, E, true); else VR_L2(M, E, false); } while (0)
+    if (mode == VR_MIP) VR_L1(VR_MIP, false);
+    else if (ert) VR_L1(VR_EA, true);
+    else VR_L1(VR_EA, false);
+#undef VR_L1
+#undef VR_L2
+#undef VR_L3
+}
+
+void launch_transpose_xz(const float *in, float *out, int nx, int ny, int nz, cudaStream_t st)
+{
+    // gridDim.y, .z <= 65535: nz <= 2^21 and ny <= 65535 per launch; larger y extents go slab by slab
+    for (int y0 = 0; y0 < ny; y0 += 65535) {
+        const int yn = ny - y0 < 65535 ? ny - y0 : 65535;
+        const dim3 g((unsigned)((nx + 31) / 32), (unsigned)((nz + 31) / 32), (unsigned)yn);
+        vr_launch(k_transpose_xz, g, 256, 0, st, in + (long long)y0 * nx, out + (long long)y0 * nz, nx, ny, nz);
+    }
+}
+
+}  // namespace vr

@@ -3,8 +3,10 @@
 // nothing can be contracted or reassociated by the compiler: __fmaf_rn is one fused multiply-add,
 // everything else is a separately rounded IEEE-754 binary32 operation, denormals kept.
 #pragma once
+#ifndef VR_SIMT_HOST               // tests/simt/simt_host.h (force-included by the host emulation build) stands in
 #include <cuda_runtime.h>
 #include <math_constants.h>
+#endif
 #include <stdint.h>
 
 namespace vr {
@@ -19,6 +21,9 @@ __device__ __forceinline__ float lerp_ee(float a, float b, float f)
 // (a.x*b.x + c.x, a.y*b.y + c.y).  Same results as two __fmaf_rn; halves the issue slots of the lerps.
 __device__ __forceinline__ float2 fma2_rn(float2 a, float2 b, float2 c)
 {
+#ifdef VR_SIMT_HOST
+    return make_float2(__fmaf_rn(a.x, b.x, c.x), __fmaf_rn(a.y, b.y, c.y));
+#else
     unsigned long long ua, ub, uc, ud;
     asm("mov.b64 %0, {%1, %2};" : "=l"(ua) : "f"(a.x), "f"(a.y));
     asm("mov.b64 %0, {%1, %2};" : "=l"(ub) : "f"(b.x), "f"(b.y));
@@ -27,6 +32,7 @@ __device__ __forceinline__ float2 fma2_rn(float2 a, float2 b, float2 c)
     float2 d;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(ud));
     return d;
+#endif
 }
 
 // exact-ends lerp of two pairs with one fraction: (L(a.x,b.x,f), L(a.y,b.y,f))
@@ -87,7 +93,10 @@ __device__ __forceinline__ bool make_ray(const CamK &c, int nx, int ny, int nz, 
     }
     if (!(t_exit > t_enter)) hit = false;
     r.t_first = __fmaf_rn(0.5f, c.step, t_enter);
-    r.t_exit = t_exit;
+    // C.2 defines samples for k < 2^24 only ((float)k must be exact): the march loops end at that k at the
+    // latest, whatever the step, and a direction that is not finite (g = 0: t_exit = +inf or NaN) is a miss
+    if (!(t_exit < CUDART_INF_F)) hit = false;
+    r.t_exit = fminf(t_exit, __fmaf_rn(16777216.0f, c.step, r.t_first));
     return hit;
 }
 

@@ -226,7 +226,7 @@ void launch_march_full(int mode, bool ert, const CamK &cam, const VolK &vol, con
 {
     const dim3 g = tiles(cam.width, cam.height);
     const bool wide = needs_wide(vol);
-#define VR_LAUNCH(M, E, Wd) k_march_full<M, E, Wd><<<g, kThreads, 0, st>>>(cam, vol, tf, image, pitch_f)
+#define VR_LAUNCH(M, E, Wd) vr_launch(k_march_full<M, E, Wd>, g, kThreads, 0, st, cam, vol, tf, image, pitch_f)
     if (mode == VR_MIP) { if (wide) VR_LAUNCH(VR_MIP, false, true); else VR_LAUNCH(VR_MIP, false, false); }
     else if (ert) { if (wide) VR_LAUNCH(VR_EA, true, true); else VR_LAUNCH(VR_EA, true, false); }
     else { if (wide) VR_LAUNCH(VR_EA, false, true); else VR_LAUNCH(VR_EA, false, false); }
@@ -237,7 +237,7 @@ void launch_march_bricks(int mode, bool wide, const CamK &cam, const VolK &vol, 
                          const WorkK *work, int n_work, float *arena, cudaStream_t st)
 {
     if (n_work <= 0) return;
-#define VR_LAUNCH(M, Wd) k_march_bricks<M, Wd><<<n_work, kThreads, 0, st>>>(cam, vol, tf, bricks, work, arena)
+#define VR_LAUNCH(M, Wd) vr_launch(k_march_bricks<M, Wd>, n_work, kThreads, 0, st, cam, vol, tf, bricks, work, arena)
     if (mode == VR_MIP) { if (wide) VR_LAUNCH(VR_MIP, true); else VR_LAUNCH(VR_MIP, false); }
     else { if (wide) VR_LAUNCH(VR_EA, true); else VR_LAUNCH(VR_EA, false); }
 #undef VR_LAUNCH
@@ -247,15 +247,15 @@ void launch_composite(int mode, const CamK &cam, const BrickK *bricks, BinsK bin
                       long long pitch_f, cudaStream_t st)
 {
     const dim3 g((cam.width + 15) / 16, (cam.height + 15) / 16);
-    if (mode == VR_MIP) k_composite<VR_MIP><<<g, 256, 0, st>>>(cam.width, cam.height, bricks, bins, arena, image, pitch_f);
-    else k_composite<VR_EA><<<g, 256, 0, st>>>(cam.width, cam.height, bricks, bins, arena, image, pitch_f);
+    if (mode == VR_MIP) vr_launch(k_composite<VR_MIP>, g, 256, 0, st, cam.width, cam.height, bricks, bins, arena, image, pitch_f);
+    else vr_launch(k_composite<VR_EA>, g, 256, 0, st, cam.width, cam.height, bricks, bins, arena, image, pitch_f);
 }
 
 void launch_chain_init(int mode, int W, int H, float *image, long long pitch_f, cudaStream_t st)
 {
     const dim3 g((W + 31) / 32, (H + 7) / 8);
-    if (mode == VR_MIP) k_chain_init<VR_MIP><<<g, 256, 0, st>>>(W, H, image, pitch_f);
-    else k_chain_init<VR_EA><<<g, 256, 0, st>>>(W, H, image, pitch_f);
+    if (mode == VR_MIP) vr_launch(k_chain_init<VR_MIP>, g, 256, 0, st, W, H, image, pitch_f);
+    else vr_launch(k_chain_init<VR_EA>, g, 256, 0, st, W, H, image, pitch_f);
 }
 
 void launch_chain_brick(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, const BrickK &brick,
@@ -266,7 +266,7 @@ void launch_chain_brick(int mode, bool ert, const CamK &cam, const VolK &vol, co
     VolK V = vol;
     V.base = brick.base; V.sy = brick.sy; V.sz = brick.sz; V.ox = brick.ox; V.oy = brick.oy; V.oz = brick.oz;
     const bool wide = (unsigned long long)V.sz * (unsigned long long)(V.sz / (V.sy ? V.sy : 1) + 2) > 0xffffffffull;   // slot of E^3 elements
-#define VR_LAUNCH(M, E, Wd) k_chain_brick<M, E, Wd><<<g, kThreads, 0, st>>>(cam, V, tf, brick, image, pitch_f)
+#define VR_LAUNCH(M, E, Wd) vr_launch(k_chain_brick<M, E, Wd>, g, kThreads, 0, st, cam, V, tf, brick, image, pitch_f)
     if (mode == VR_MIP) { if (wide) VR_LAUNCH(VR_MIP, false, true); else VR_LAUNCH(VR_MIP, false, false); }
     else if (ert) { if (wide) VR_LAUNCH(VR_EA, true, true); else VR_LAUNCH(VR_EA, true, false); }
     else { if (wide) VR_LAUNCH(VR_EA, false, true); else VR_LAUNCH(VR_EA, false, false); }
@@ -276,7 +276,7 @@ void launch_chain_brick(int mode, bool ert, const CamK &cam, const VolK &vol, co
 void launch_chain_finish(int W, int H, float *image, long long pitch_f, cudaStream_t st)
 {
     const dim3 g((W + 31) / 32, (H + 7) / 8);
-    k_chain_finish<<<g, 256, 0, st>>>(W, H, image, pitch_f);
+    vr_launch(k_chain_finish, g, 256, 0, st, W, H, image, pitch_f);
 }
 
 }  // namespace vr

@@ -35,10 +35,14 @@ __device__ __forceinline__ float dec_f(unsigned int u)
 
 __device__ __forceinline__ float4 ld_stream4(const float4 *p)
 {
+#ifdef VR_SIMT_HOST
+    return *p;
+#else
     float4 r;
     asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
                  : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
     return r;
+#endif
 }
 
 struct Acc {                                   // per-thread running state
@@ -143,7 +147,7 @@ template <bool MINMAX, bool HIST>
 __global__ void __launch_bounds__(kThreads, 2)
 k_reduce_flat(const float *__restrict__ v, unsigned long long n, uint32_t nbins, SummaryScratch *s)
 {
-    extern __shared__ unsigned int smem[];
+    VR_DYN_SHARED(unsigned int, smem);
     const HistCtx hc = hist_begin<HIST>(s, nbins, smem);
     Acc a = { CUDART_INF_F, -CUDART_INF_F, 0u, 0u, 0u };
     const unsigned long long n4 = n >> 2;
@@ -176,7 +180,7 @@ template <bool MINMAX, bool HIST>
 __global__ void __launch_bounds__(kThreads, 2)
 k_reduce_box(BoxK b, uint32_t nbins, SummaryScratch *s)
 {
-    extern __shared__ unsigned int smem[];
+    VR_DYN_SHARED(unsigned int, smem);
     const HistCtx hc = hist_begin<HIST>(s, nbins, smem);
     Acc a = { CUDART_INF_F, -CUDART_INF_F, 0u, 0u, 0u };
     const int lane = threadIdx.x & 31;
@@ -221,40 +225,40 @@ constexpr size_t kHistSmemBytes = kHistSmemWords * sizeof(unsigned int);
 
 }  // namespace
 
-void launch_summary_reset(SummaryScratch *s, cudaStream_t st) { k_summary_reset<<<16, 256, 0, st>>>(s); }
+void launch_summary_reset(SummaryScratch *s, cudaStream_t st) { vr_launch(k_summary_reset, 16, 256, 0, st, s); }
 
 void launch_minmax_flat(const float *v, unsigned long long n, SummaryScratch *s, int grid, cudaStream_t st)
 {
-    k_reduce_flat<true, false><<<grid, kThreads, 0, st>>>(v, n, 0u, s);
+    vr_launch(k_reduce_flat<true, false>, grid, kThreads, 0, st, v, n, 0u, s);
 }
 void launch_minmax_box(BoxK b, SummaryScratch *s, int grid, cudaStream_t st)
 {
-    k_reduce_box<true, false><<<grid, kThreads, 0, st>>>(b, 0u, s);
+    vr_launch(k_reduce_box<true, false>, grid, kThreads, 0, st, b, 0u, s);
 }
 void launch_summary_range(SummaryScratch *s, int range_mode, float lo, float hi, uint32_t nbins, cudaStream_t st)
 {
-    k_summary_range<<<1, 1, 0, st>>>(s, range_mode, lo, hi, nbins);
+    vr_launch(k_summary_range, 1, 1, 0, st, s, range_mode, lo, hi, nbins);
 }
 void launch_hist_flat(const float *v, unsigned long long n, uint32_t nbins, SummaryScratch *s, int grid, cudaStream_t st)
 {
-    k_reduce_flat<false, true><<<grid, kThreads, kHistSmemBytes, st>>>(v, n, nbins, s);
+    vr_launch(k_reduce_flat<false, true>, grid, kThreads, kHistSmemBytes, st, v, n, nbins, s);
 }
 void launch_hist_box(BoxK b, uint32_t nbins, SummaryScratch *s, int grid, cudaStream_t st)
 {
-    k_reduce_box<false, true><<<grid, kThreads, kHistSmemBytes, st>>>(b, nbins, s);
+    vr_launch(k_reduce_box<false, true>, grid, kThreads, kHistSmemBytes, st, b, nbins, s);
 }
 void launch_minmax_hist_flat(const float *v, unsigned long long n, uint32_t nbins, SummaryScratch *s, int grid,
                              cudaStream_t st)
 {
-    k_reduce_flat<true, true><<<grid, kThreads, kHistSmemBytes, st>>>(v, n, nbins, s);
+    vr_launch(k_reduce_flat<true, true>, grid, kThreads, kHistSmemBytes, st, v, n, nbins, s);
 }
 void launch_minmax_hist_box(BoxK b, uint32_t nbins, SummaryScratch *s, int grid, cudaStream_t st)
 {
-    k_reduce_box<true, true><<<grid, kThreads, kHistSmemBytes, st>>>(b, nbins, s);
+    vr_launch(k_reduce_box<true, true>, grid, kThreads, kHistSmemBytes, st, b, nbins, s);
 }
 void launch_summary_finish(const SummaryScratch *s, uint32_t nbins, vr_summary *out, cudaStream_t st)
 {
-    k_summary_finish<<<(nbins + 255) / 256, 256, 0, st>>>(s, nbins, out);
+    vr_launch(k_summary_finish, (nbins + 255) / 256, 256, 0, st, s, nbins, out);
 }
 
 }  // namespace vr

@@ -4,6 +4,12 @@ import numpy as np
 MIP_REL = 1e-6       # north_star: MIP within 1e-6 relative error (scale-relative, S17)
 EA_ABS = 1e-4        # north_star: emission-absorption RGBA within 1e-4 absolute per channel
 ERT_BOUND = (1 - 0.99) + 1e-4
+# S14: ERT-fragile pixels (some T_k within 1e-5 of the threshold) must be rarer than 0.5 % of hit pixels on the
+# configs' TF_HAZE workloads, where few rays terminate.  Under TF_OPAQUE EVERY ray terminates, and the chance that
+# one of its T_k lands within +-1e-5 of 0.01 is about 2e-5 / (0.01 alpha) ~ 0.5-1 % per ray (the oracle alone gives
+# 0.1-0.6 % on the small test views), so those tests allow 2 %.  The GPU images are bit-identical to the oracle's
+# anyway; the bound only guards the workload.
+FRAGILE_FRAC_OPAQUE = 0.02
 
 
 def check_mip(gpu: np.ndarray, ref: np.ndarray, data_scale: float):
