@@ -20,8 +20,8 @@
  * per-column max (bit-exact); P2 constant cube => A = 1-(1-a)^K; P3 bricked ==
  * unbricked; P4 min/max/hist == brute force; P5 affine cube; P6 impulse tent;
  * P7 alpha 0 / alpha 1; P8 sample counts; P9/P10 mirror symmetry; P11 ERT bound;
- * P12 f32 vs f64 distance; P13 step-halving convergence.  No function here is
- * "parity unpinned".
+ * P12 f32 vs f64 distance; P13 step-halving convergence; P14 halo layout; P15
+ * non-finite voxels in a render (S24).  No function here is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -mfma -ffp-contract=off -shared -fPIC vr_oracle.c -lm
  */

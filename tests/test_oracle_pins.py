@@ -420,3 +420,56 @@ def test_oracle_matches_its_committed_golden():
     with open(os.path.join(here, "oracle_tiny.txt")) as f:
         stored = f.read().splitlines()
     assert list(mod.lines()) == stored
+
+
+# --------------------------------------------------------------------------- P15: S24, non-finite voxels in a render
+def _nonfinite_cube():
+    v = noise_cube(11, 9, 13, seed=77).copy()       # (nz, ny, nx) = (13, 9, 11)
+    v[4, 3, 5] = np.nan
+    v[9, 7, 2] = np.inf
+    v[1, 1, 8] = -np.inf
+    return v
+
+
+def _polluted(v):
+    """Voxel-centre samples whose 8 corners (C.3: i0 = min(i, n-2), corners i0, i0+1) are not all finite.  The
+    exact-ends lerp L(a,b,f) = fma(f, b, fma(-f, a, a)) multiplies BOTH ends by a weight, so a NaN or infinite
+    corner makes the sample NaN even at weight 0 (0 * inf = NaN) — also when the infinite corner is the sampled
+    voxel itself (-0 * inf).  (No non-finite voxel of these cubes lies on a high face, where f = 1.)"""
+    nz, ny, nx = v.shape
+    bad = np.zeros(v.shape, dtype=bool)
+    for z in range(nz):
+        for y in range(ny):
+            for x in range(nx):
+                x0, y0, z0 = min(x, nx - 2), min(y, ny - 2), min(z, nz - 2)
+                bad[z, y, x] = not np.all(np.isfinite(v[z0:z0 + 2, y0:y0 + 2, x0:x0 + 2]))
+    return bad
+
+
+def test_p15_nonfinite_voxels_mip_ignores_nan_samples():
+    """S24: a NaN sample is ignored by MIP (fmaxf keeps the other operand).  Axis view at voxel centres, so every
+    sample is one voxel unless a non-finite corner turns it into NaN: expected = brute-force column max over the
+    unpolluted voxels."""
+    v = _nonfinite_cube()
+    bad = _polluted(v)
+    r = O.render(v, W.ortho_axis_camera((11, 9, 13), 2, +1, step=1.0), O.MIP)
+    want = np.where(bad, -np.inf, v).max(axis=0)
+    assert np.array_equal(r.image, want)
+    assert bad.sum() >= 24 and np.isfinite(r.image).all()          # 3 voxels x >= 8 base cells; every column keeps clean samples
+    assert not np.isnan(r.image).any()
+
+
+def test_p15_nonfinite_voxels_ea_classifies_nan_as_entry_zero():
+    """S24 / C.4: u = sat(fma(s, scale, bias)) maps a NaN sample to table entry 0 (+inf to entry 255, -inf to 0).
+    With a table whose alpha is 1 only at entry 0 (and 0 elsewhere, exact), a ray is opaque after its first
+    NaN / -inf / below-range sample and transparent before it: A = 1 exactly where the column holds such a sample."""
+    v = np.abs(_nonfinite_cube()) + 1.0            # finite voxels in [1, ~6]; nan stays nan, inf stays +inf
+    v[1, 1, 8] = -np.inf
+    tf = np.zeros((256, 4), dtype=np.float32)
+    tf[0] = (0.25, 0.5, 0.75, 1.0)
+    vmin, vmax = 0.0, 8.0                           # finite samples land on u >= 1/8 -> entries >= 31: alpha exactly 0
+    r = O.render(v, W.ortho_axis_camera((11, 9, 13), 2, +1, step=1.0), O.EA, tf, vmin, vmax)
+    bad = _polluted(v)
+    want_a = bad.any(axis=0).astype(np.float32)
+    assert np.array_equal(r.image[..., 3], want_a)
+    assert np.array_equal(r.image[..., 0], 0.25 * want_a) and np.array_equal(r.image[..., 2], 0.75 * want_a)

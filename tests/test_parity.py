@@ -455,3 +455,32 @@ def test_cfg4_full_size_sampled():
     if avail < 80 << 30:
         pytest.skip("needs 80 GB of host memory for the cube the oracle reads")
     _full_size_case(4, views=(5, 12), summary_exact=True, stride=16)
+
+
+# ------------------------------------------------------------------ S24: non-finite voxels in a rendered cube
+def test_nonfinite_voxels_render_like_the_oracle(be):
+    """FITS blanks: NaN and +-Inf voxels.  A NaN sample classifies as table entry 0 and is ignored by MIP (C.4, C.6,
+    S24; pinned for the oracle by P15); every render path must reproduce the oracle bit for bit, NaN for NaN."""
+    n = (40, 33, 27)
+    v = W.make_cube(W.Recipe(*n, seed=5, n_sources=2)).copy()
+    v[0, 0, 0], v[5, 6, 7], v[20, 30, 35], v[13, 1, 2], v[14, 16, 20] = np.nan, np.inf, -np.inf, np.nan, np.nan
+    s = O.minmax_hist(v)
+    tf = W.tf_opaque(n, 0.5)
+    c = np.array(n) / 2
+    cams = [W.perspective_camera(c + np.array([0.4, 0.5, 1.7]) * 40, c, (0, 1, 0), 40.0, 70, 50, step=0.5),
+            W.perspective_camera(c + np.array([1.8, 0.3, -0.4]) * 40, c, (0, 1, 0), 40.0, 70, 50, step=0.5, ert_alpha=0.99),
+            W.ortho_axis_camera(n, 2, +1, step=1.0)]
+    for path, brick, flags in ((0, 0, 0), (1, 0, 0), (0, 16, W.cameras.VR_SORT_LAST)):
+        with vr.Volume(be.dev(v), n, brick=brick) as vol:
+            vol.set_option(vr.VR_OPT_RENDER_PATH, path)
+            vol.set_transfer_function(tf, s.vmin, s.vmax)
+            for cam in cams:
+                if flags and cam.ert_alpha:
+                    continue
+                cam = cam.with_(flags=flags)
+                om = O.render(v, cam, O.MIP, brick=brick if flags else 0)
+                oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax, brick=brick if flags else 0)
+                gm = render(be, vol, cam, vr.VR_MIP)
+                ge = render(be, vol, cam, vr.VR_EA)
+                assert np.array_equal(gm, om.image, equal_nan=True) and np.array_equal(ge, oe.image, equal_nan=True)
+                assert not np.isnan(om.image).any()          # MIP never returns NaN (fmaxf drops it)
