@@ -48,6 +48,11 @@ class _Head(C.Structure):
                 ("n_below", C.c_uint64), ("n_above", C.c_uint64)]
 
 
+class _Stats(C.Structure):
+    _fields_ = [("n_finite", C.c_uint64), ("n_nonfinite", C.c_uint64), ("mean", C.c_double), ("stddev", C.c_double),
+                ("median", C.c_float), ("pad", C.c_float)]
+
+
 def _load():
     global _lib
     if _lib is None:
@@ -57,6 +62,9 @@ def _load():
         lib.oracle_minmax_hist.restype = C.c_int
         lib.oracle_minmax_hist.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
                                            C.c_uint32, C.c_void_p, C.POINTER(_Head), C.c_void_p]
+        lib.oracle_statistics.restype = C.c_int
+        lib.oracle_statistics.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
+                                          C.POINTER(_Stats)]
         lib.oracle_num_threads.restype = C.c_int
         _lib = lib
     return _lib
@@ -167,3 +175,26 @@ def minmax_hist(vol: np.ndarray, nbins: int = 256, range_=None, layout: int = LI
         raise ValueError(f"oracle_minmax_hist failed: {rc}")
     return Summary(np.float32(head.vmin), np.float32(head.vmax), int(head.n_nonfinite), int(head.n_below),
                    int(head.n_above), counts)
+
+
+@dataclass
+class Statistics:
+    n_finite: int
+    n_nonfinite: int
+    mean: float                  # double
+    stddev: float                # double, population
+    median: np.float32           # lower median, a data value
+
+
+def statistics(vol: np.ndarray, layout: int = LINEAR, layout_brick: int = 0, dims=None) -> Statistics:
+    lib = _load()
+    assert vol.dtype == np.float32 and vol.flags["C_CONTIGUOUS"]
+    if layout == LINEAR:
+        nz, ny, nx = vol.shape
+    else:
+        nx, ny, nz = dims
+    st = _Stats()
+    rc = lib.oracle_statistics(vol.ctypes.data, nx, ny, nz, layout, layout_brick, C.byref(st))
+    if rc != 0:
+        raise ValueError(f"oracle_statistics failed: {rc}")
+    return Statistics(int(st.n_finite), int(st.n_nonfinite), float(st.mean), float(st.stddev), np.float32(st.median))

@@ -494,6 +494,82 @@ ORACLE_EXPORT int oracle_minmax_hist(const float *vol, uint32_t nx, uint32_t ny,
     return 0;
 }
 
+/* ------------------------------------------------------------------ */
+/* C.13: mean, standard deviation, median over finite voxels           */
+/* (the "global view" statistics of PAPER.md:L66; readings S35-S37)    */
+/* ------------------------------------------------------------------ */
+typedef struct {
+    uint64_t n_finite, n_nonfinite;
+    double mean;        /* S35: sum(v)/n over finite voxels, accumulated in double */
+    double stddev;      /* S36: POPULATION standard deviation sqrt(sum((v-mean)^2)/n), second pass, double */
+    float median;       /* S37: LOWER median = the element of rank floor((n-1)/2) (0-based) of the finite voxels
+                           sorted by value, -0 before +0 (IEEE totalOrder); a data value, so bit-exact */
+    float pad;
+} oracle_stats;
+
+/* order-preserving key of a float: a < b (totalOrder) <=> key(a) < key(b) */
+static inline uint32_t total_order_key(float f)
+{
+    uint32_t b; memcpy(&b, &f, 4);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+static int cmp_key(const void *a, const void *b)
+{
+    uint32_t x = *(const uint32_t *)a, y = *(const uint32_t *)b;
+    return x < y ? -1 : x > y ? 1 : 0;
+}
+
+/* Plain definition: gather the finite voxels (halo voxels of a bricked layout excluded), Neumaier-compensated
+ * double sums in voxel order for the two moments, qsort of the keys for the median. */
+ORACLE_EXPORT int oracle_statistics(const float *vol, uint32_t nx, uint32_t ny, uint32_t nz, uint32_t layout,
+                                    uint32_t layout_brick, oracle_stats *out)
+{
+    if (!vol || !out || !nx || !ny || !nz) return -1;
+    volume V = { vol, nx, ny, nz, (int)layout, (int64_t)layout_brick, 0, 0 };
+    if (V.layout == ORACLE_BRICKED_HALO1) {
+        if (!V.B) return -5;
+        V.nbx = (V.nx + V.B - 1) / V.B; V.nby = (V.ny + V.B - 1) / V.B;
+    }
+    const uint64_t N = (uint64_t)nx * ny * nz;
+    uint32_t *keys = (uint32_t *)malloc(sizeof(uint32_t) * (size_t)N);
+    if (!keys) return -7;
+    uint64_t n = 0, nonfinite = 0;
+    double sum = 0.0, comp = 0.0;
+    for (int64_t z = 0; z < V.nz; ++z)
+        for (int64_t y = 0; y < V.ny; ++y)
+            for (int64_t x = 0; x < V.nx; ++x) {
+                float v = vox_corner(&V, x, y, z, 0, 0, 0);
+                if (!isfinite(v)) { ++nonfinite; continue; }
+                keys[n++] = total_order_key(v);
+                double t = sum + (double)v;                       /* Neumaier */
+                comp += fabs(sum) >= fabs((double)v) ? (sum - t) + (double)v : ((double)v - t) + sum;
+                sum = t;
+            }
+    out->n_finite = n; out->n_nonfinite = nonfinite;
+    out->mean = 0.0; out->stddev = 0.0; out->median = 0.0f; out->pad = 0.0f;
+    if (n == 0) { free(keys); out->mean = NAN; out->stddev = NAN; out->median = NAN; return 0; }
+    const double mean = (sum + comp) / (double)n;
+    double ss = 0.0, sc = 0.0;
+    for (int64_t z = 0; z < V.nz; ++z)
+        for (int64_t y = 0; y < V.ny; ++y)
+            for (int64_t x = 0; x < V.nx; ++x) {
+                float v = vox_corner(&V, x, y, z, 0, 0, 0);
+                if (!isfinite(v)) continue;
+                double d = (double)v - mean, q = d * d;
+                double t = ss + q;
+                sc += ss >= q ? (ss - t) + q : (q - t) + ss;
+                ss = t;
+            }
+    out->mean = mean;
+    out->stddev = sqrt((ss + sc) / (double)n);
+    qsort(keys, (size_t)n, sizeof(uint32_t), cmp_key);
+    uint32_t k = keys[(n - 1) / 2];
+    uint32_t bits = (k & 0x80000000u) ? (k & 0x7fffffffu) : ~k;
+    memcpy(&out->median, &bits, 4);
+    free(keys);
+    return 0;
+}
+
 ORACLE_EXPORT int oracle_num_threads(void)
 {
     int n = 1;

@@ -473,3 +473,50 @@ def test_p15_nonfinite_voxels_ea_classifies_nan_as_entry_zero():
     want_a = bad.any(axis=0).astype(np.float32)
     assert np.array_equal(r.image[..., 3], want_a)
     assert np.array_equal(r.image[..., 0], 0.25 * want_a) and np.array_equal(r.image[..., 2], 0.75 * want_a)
+
+
+# --------------------------------------------------------------------------- P16: mean / standard deviation / median
+def test_p16_statistics_closed_forms():
+    """C.13 (S35-S37).  Integers 0..255, each 32 times: mean 127.5, population variance (256^2-1)/12, lower median
+    127 (rank (8192-1)//2 = 4095 -> value 4095 // 32).  Constant cube: std 0, median c.  Two-point cube."""
+    k = np.repeat(np.arange(256), 32).astype(np.float32)
+    RNG.shuffle(k)
+    s = O.statistics(k.reshape(8, 32, 32))
+    assert s.n_finite == 8192 and s.n_nonfinite == 0
+    assert s.mean == 127.5 and abs(s.stddev - math.sqrt((256 ** 2 - 1) / 12)) < 1e-12 and s.median == 127.0
+    c = np.full((5, 6, 7), -3.25, dtype=np.float32)
+    s = O.statistics(c)
+    assert s.mean == -3.25 and s.stddev == 0.0 and s.median == np.float32(-3.25)
+    two = np.array([1.0] * 30 + [5.0] * 30, dtype=np.float32).reshape(3, 4, 5)     # even n: LOWER median
+    s = O.statistics(two)
+    assert s.mean == 3.0 and s.stddev == 2.0 and s.median == 1.0
+    two[0, 0, 0] = 5.0                                                              # 29 ones, 31 fives
+    assert O.statistics(two).median == 5.0
+
+
+def test_p16_statistics_match_numpy_and_sorting():
+    """Against library routines on a noise+sources cube with planted non-finite voxels: float64 mean / std of numpy
+    (pairwise summation) within 1e-13 relative; the median is EXACTLY the element of rank (n-1)//2 of np.sort."""
+    v = W.make_cube(W.Recipe(37, 29, 41, seed=8, n_sources=3)).copy()
+    v[3, 4, 5], v[7, 7, 7], v[20, 1, 30] = np.nan, np.inf, -np.inf
+    s = O.statistics(v)
+    f = v[np.isfinite(v)].astype(np.float64)
+    assert s.n_finite == f.size and s.n_nonfinite == 3
+    assert abs(s.mean - f.mean()) <= 1e-13 * np.abs(f).mean()
+    assert abs(s.stddev - f.std()) <= 1e-13 * f.std()
+    assert s.median == np.sort(v[np.isfinite(v)])[(f.size - 1) // 2]
+    # n even and odd, and the signed-zero order (-0 sorts before +0)
+    z = np.array([0.0, -0.0, -0.0, 0.0, 1.0, -1.0, -0.0, 2.0], dtype=np.float32).reshape(2, 2, 2)   # sorted: -1 -0 -0 -0 +0 +0 1 2
+    m = O.statistics(z).median
+    assert m == 0.0 and np.signbit(m)                # rank 3 is the last -0
+    z[0, 0, 1] = 0.0                                 # sorted: -1 -0 -0 +0 +0 +0 1 2 -> rank 3 is +0
+    m = O.statistics(z).median
+    assert m == 0.0 and not np.signbit(m)
+
+
+def test_p16_statistics_bricked_halo_layout_equals_linear():
+    v = W.make_cube(W.Recipe(21, 18, 26, seed=9, n_sources=2))
+    t = W.retile_halo(v, 8)
+    a, b = O.statistics(v), O.statistics(t, layout=O.BRICKED_HALO1, layout_brick=8, dims=(21, 18, 26))
+    assert a.n_finite == b.n_finite and a.median == b.median
+    assert abs(a.mean - b.mean) < 1e-14 and abs(a.stddev - b.stddev) < 1e-14      # same values, another voxel order
