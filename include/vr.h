@@ -197,6 +197,33 @@ VR_API vr_status vr_minmax_histogram(vr_volume *vol, uint32_t nbins, const float
                                      uint32_t out_location, void *stream);
 
 /* ------------------------------------------------------------------------------------------
+ * vr_statistics — the multi-pass "global view" statistics of the whole cube (
+ * PAPER.md:L66 "global view data analysis tasks ... [like] median and standard deviation", which need
+ * every voxel and several passes over the data; readings S35-S37 of DESIGN.md §3).  Over the voxels
+ * with isfinite(v) (n_finite of them; n_nonfinite counts the rest; halo voxels of a bricked layout are
+ * not counted):
+ *   mean     sum(v) / n_finite, accumulated in float64 (compensated; S35).
+ *   stddev   POPULATION standard deviation sqrt(sum((v - mean)^2) / n_finite), second pass, float64 (S36).
+ *   median   the LOWER median: the voxel value of rank floor((n_finite - 1) / 2) (0-based) in ascending
+ *            IEEE totalOrder (-0 before +0).  A data value, found exactly by a 4-pass radix select on the
+ *            order-preserving bit pattern (S37); no sorting, no approximation.
+ *   n_finite == 0: mean, stddev and median are NaN.
+ * Five streams of the cube (4 B/voxel each) enqueued on `stream`, nothing read back in between; float64
+ * sums are deterministic for a given device (fixed reduction order), and equal to any other correct
+ * summation within a few units of 1e-16 * mean(|v|).  Out-of-core volumes ride the brick streamer.
+ *   out   DEVICE (out_location VR_DEVICE) or pinned HOST (VR_HOST_PINNED), 8-byte aligned.
+ * Errors: VR_ERR_INVALID_ARG, VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+    uint64_t n_finite, n_nonfinite;
+    double mean, stddev;
+    float median;
+    uint32_t reserved;
+} vr_statistics_result;
+
+VR_API vr_status vr_statistics(vr_volume *vol, vr_statistics_result *out, uint32_t out_location, void *stream);
+
+/* ------------------------------------------------------------------------------------------
  * vr_get_stats — counters of the last vr_render / vr_minmax_histogram on this handle
  * (SURVEY.md §5 "metrics"): host-side values only, no synchronisation.
  * ------------------------------------------------------------------------------------------ */

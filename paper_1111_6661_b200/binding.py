@@ -57,8 +57,13 @@ class vr_stats(C.Structure):
                 ("zfast_copy", C.c_uint32), ("reserved", C.c_uint32)]
 
 
+class vr_statistics_result(C.Structure):
+    _fields_ = [("n_finite", C.c_uint64), ("n_nonfinite", C.c_uint64), ("mean", C.c_double), ("stddev", C.c_double),
+                ("median", C.c_float), ("reserved", C.c_uint32)]
+
+
 EXPORTS = ("vr_create_volume", "vr_destroy_volume", "vr_set_transfer_function", "vr_render",
-           "vr_minmax_histogram", "vr_get_stats", "vr_set_option", "vr_last_error", "vr_version")
+           "vr_minmax_histogram", "vr_statistics", "vr_get_stats", "vr_set_option", "vr_last_error", "vr_version")
 
 _lib = None
 
@@ -80,6 +85,8 @@ def _declare(lib):
         lib.vr_render.argtypes = [C.c_void_p, C.POINTER(vr_camera), C.c_int, C.POINTER(vr_image), C.c_void_p]
         lib.vr_minmax_histogram.restype = C.c_int
         lib.vr_minmax_histogram.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+        lib.vr_statistics.restype = C.c_int
+        lib.vr_statistics.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
         lib.vr_get_stats.restype = C.c_int
         lib.vr_get_stats.argtypes = [C.c_void_p, C.POINTER(vr_stats)]
         lib.vr_set_option.restype = C.c_int
@@ -135,6 +142,10 @@ def make_camera(cam) -> vr_camera:
 def summary_dtype(nbins: int) -> np.dtype:
     return np.dtype([("vmin", np.float32), ("vmax", np.float32), ("n_nonfinite", np.uint64),
                      ("n_below", np.uint64), ("n_above", np.uint64), ("counts", np.uint64, (nbins,))])
+
+
+STATISTICS_DTYPE = np.dtype([("n_finite", np.uint64), ("n_nonfinite", np.uint64), ("mean", np.float64),
+                             ("stddev", np.float64), ("median", np.float32), ("reserved", np.uint32)])
 
 
 class Volume:
@@ -221,6 +232,28 @@ class Volume:
             torch.cuda.current_stream().synchronize()
             buf = buf.cpu()
         return np.frombuffer(buf.numpy().tobytes()[: 32 + 8 * nbins], dtype=summary_dtype(nbins))[0]
+
+    # -- vr_statistics
+    def statistics(self, out=None, stream=None):
+        """Enqueue the mean / standard deviation / median passes.  `out`: uint8 tensor of 40 bytes (CUDA or pinned
+        CPU); allocated on the device if None.  Returns the tensor; see read_statistics()."""
+        import torch
+        nbytes = C.sizeof(vr_statistics_result)
+        if out is None:
+            out = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        assert out.numel() * out.element_size() >= nbytes
+        _check(load().vr_statistics(self._h, out.data_ptr(), VR_DEVICE if out.is_cuda else VR_HOST_PINNED,
+                                    _stream_ptr(stream)))
+        return out
+
+    @staticmethod
+    def read_statistics(buf):
+        """Synchronise and decode a statistics buffer into a numpy record."""
+        import torch
+        if buf.is_cuda:
+            torch.cuda.current_stream().synchronize()
+            buf = buf.cpu()
+        return np.frombuffer(buf.numpy().tobytes()[: C.sizeof(vr_statistics_result)], dtype=STATISTICS_DTYPE)[0]
 
     # -- vr_set_option
     def set_option(self, option: int, value: int):

@@ -97,6 +97,8 @@ struct vr_volume {
     // scratch
     SummaryScratch *d_sum = nullptr;
     vr_summary *d_sum_out = nullptr;          // staging for host outputs
+    StatScratch *d_stat = nullptr;            // vr_statistics (allocated on first use)
+    vr_statistics_result *d_stat_out = nullptr;
     DevBuf<float> arena, host_image;
 
     // lane-mapped path: the library's z-fastest copy of a resident linear volume (vr_lanes.cu)
@@ -130,6 +132,8 @@ static void free_volume(vr_volume *v)
     if (v->d_tf) cudaFree(v->d_tf);
     if (v->d_sum) cudaFree(v->d_sum);
     if (v->d_sum_out) cudaFree(v->d_sum_out);
+    if (v->d_stat) cudaFree(v->d_stat);
+    if (v->d_stat_out) cudaFree(v->d_stat_out);
     if (v->zfast) cudaFree(v->zfast);
     if (v->zfast_ev) cudaEventDestroy(v->zfast_ev);
     v->arena.release();
@@ -474,6 +478,43 @@ static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam,
     return VR_OK;
 }
 
+// ------------------------------------------------------------------ one pass over every voxel (A1, A2, statistics)
+// VR_LINEAR: one launch on the flat array; VR_BRICKED_HALO1: one launch per brick on its box without the halo,
+// out of core through the brick streamer (uploads of the next bricks overlap the kernel of the current one).
+template <typename Flat, typename Box>
+static vr_status sweep_volume(vr_volume *v, cudaStream_t st, int grid, Flat &&flat, Box &&box_fn)
+{
+    if (v->desc.layout == VR_LINEAR) {
+        flat(v->dev_data, (unsigned long long)v->n_vox, grid);
+        v->stats.kernel_launches += 1;
+        return VR_OK;
+    }
+    const uint32_t n[3] = { v->desc.nx, v->desc.ny, v->desc.nz };
+    for (uint32_t bz = 0; bz < v->nb[2]; ++bz)
+        for (uint32_t by = 0; by < v->nb[1]; ++by)
+            for (uint32_t bx = 0; bx < v->nb[0]; ++bx) {
+                const uint64_t id = brick_id(v, bx, by, bz);
+                BoxK box;
+                uint32_t slot = 0;
+                if (v->out_of_core) {
+                    const float *ptr;
+                    vr_status rc = stream_brick_acquire(v, id, st, &ptr, &slot);
+                    if (rc != VR_OK) return rc;
+                    box.base = ptr;
+                } else box.base = v->dev_data + id * v->brick_elems;
+                box.sy = v->E; box.sz = (long long)v->E * v->E;
+                const uint32_t bb[3] = { bx, by, bz };
+                int ext[3];
+                for (int a = 0; a < 3; ++a) ext[a] = (int)std::min(v->B, n[a] - bb[a] * v->B);   // halo excluded
+                box.ex = ext[0]; box.ey = ext[1]; box.ez = ext[2];
+                const int bgrid = (int)std::max<long long>(1, std::min<long long>(grid, ((long long)box.ey * box.ez + 15) / 16));
+                box_fn(box, bgrid);
+                v->stats.kernel_launches += 1;
+                if (v->out_of_core) { vr_status rc = stream_brick_release(v, slot, st); if (rc != VR_OK) return rc; }
+            }
+    return VR_OK;
+}
+
 }  // namespace vr
 
 // ====================================================================== C ABI
@@ -683,48 +724,69 @@ VR_API vr_status vr_minmax_histogram(vr_volume *v, uint32_t nbins, const float *
     launch_summary_reset(S, st);
     v->stats.kernel_launches += 1;
     const int n_pass = range ? 1 : 2;
-    const uint32_t n[3] = { v->desc.nx, v->desc.ny, v->desc.nz };
     for (int pass = 0; pass < n_pass; ++pass) {
         // pass 0: min/max (+ histogram when the caller gave the range); pass 1: histogram over [min,max]
         if (range && pass == 0) { launch_summary_range(S, 1, lo, hi, nbins, st); v->stats.kernel_launches += 1; }
         if (pass == 1) { launch_summary_range(S, 0, 0.0f, 0.0f, nbins, st); v->stats.kernel_launches += 1; }
-        if (v->desc.layout == VR_LINEAR) {
-            if (pass == 1) launch_hist_flat(v->dev_data, v->n_vox, nbins, S, grid, st);
-            else if (range) launch_minmax_hist_flat(v->dev_data, v->n_vox, nbins, S, grid, st);
-            else launch_minmax_flat(v->dev_data, v->n_vox, S, grid, st);
-            v->stats.kernel_launches += 1;
-        } else {
-            for (uint32_t bz = 0; bz < v->nb[2]; ++bz)
-                for (uint32_t by = 0; by < v->nb[1]; ++by)
-                    for (uint32_t bx = 0; bx < v->nb[0]; ++bx) {
-                        const uint64_t id = brick_id(v, bx, by, bz);
-                        BoxK box;
-                        uint32_t slot = 0;
-                        if (v->out_of_core) {
-                            const float *ptr;
-                            rc = stream_brick_acquire(v, id, st, &ptr, &slot);
-                            if (rc != VR_OK) return rc;
-                            box.base = ptr;
-                        } else box.base = v->dev_data + id * v->brick_elems;
-                        box.sy = v->E; box.sz = (long long)v->E * v->E;
-                        const uint32_t bb[3] = { bx, by, bz };
-                        int ext[3];
-                        for (int a = 0; a < 3; ++a) ext[a] = (int)std::min(v->B, n[a] - bb[a] * v->B);   // halo excluded
-                        box.ex = ext[0]; box.ey = ext[1]; box.ez = ext[2];
-                        const int bgrid = (int)std::min<long long>(grid, ((long long)box.ey * box.ez + 15) / 16);
-                        if (pass == 1) launch_hist_box(box, nbins, S, bgrid, st);
-                        else if (range) launch_minmax_hist_box(box, nbins, S, bgrid, st);
-                        else launch_minmax_box(box, S, bgrid, st);
-                        v->stats.kernel_launches += 1;
-                        if (v->out_of_core) { rc = stream_brick_release(v, slot, st); if (rc != VR_OK) return rc; }
-                    }
-        }
+        rc = sweep_volume(v, st, grid,
+            [&](const float *p, unsigned long long n, int g) {
+                if (pass == 1) launch_hist_flat(p, n, nbins, S, g, st);
+                else if (range) launch_minmax_hist_flat(p, n, nbins, S, g, st);
+                else launch_minmax_flat(p, n, S, g, st);
+            },
+            [&](const BoxK &box, int g) {
+                if (pass == 1) launch_hist_box(box, nbins, S, g, st);
+                else if (range) launch_minmax_hist_box(box, nbins, S, g, st);
+                else launch_minmax_box(box, S, g, st);
+            });
+        if (rc != VR_OK) return rc;
     }
     if (out_location == VR_DEVICE) launch_summary_finish(S, nbins, out, st);
     else {
         launch_summary_finish(S, nbins, v->d_sum_out, st);
         VR_CUDA(cudaMemcpyAsync(out, v->d_sum_out, VR_SUMMARY_BYTES(nbins), cudaMemcpyDeviceToHost, st));
         v->stats.d2h_bytes += VR_SUMMARY_BYTES(nbins);
+    }
+    v->stats.kernel_launches += 1;
+    VR_CUDA(cudaGetLastError());
+    v->stats.total_kernel_launches += v->stats.kernel_launches;
+    return VR_OK;
+}
+
+VR_API vr_status vr_statistics(vr_volume *v, vr_statistics_result *out, uint32_t out_location, void *stream)
+{
+    g_err[0] = 0;
+    VR_REQUIRE(v && out, "vr_statistics: NULL argument");
+    VR_REQUIRE(out_location == VR_DEVICE || out_location == VR_HOST_PINNED, "bad out_location %u", out_location);
+    VR_REQUIRE(((uintptr_t)out & 7u) == 0, "out must be 8-byte aligned");
+    VR_CUDA(cudaSetDevice(v->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    v->stats.kernel_launches = 0; v->stats.h2d_bytes = 0; v->stats.d2h_bytes = 0;
+    vr_status rc = ensure_mirror(v, st);
+    if (rc != VR_OK) return rc;
+    if (!v->d_stat) {
+        VR_CUDA(cudaMalloc(&v->d_stat, sizeof(StatScratch)));
+        VR_CUDA(cudaMalloc(&v->d_stat_out, sizeof(vr_statistics_result)));
+    }
+    const int grid = std::min(v->sm_count * 2, kStatMaxGrid);
+    StatScratch *S = v->d_stat;
+    launch_stat_reset(S, st);
+    v->stats.kernel_launches += 1;
+    // pass 0: count, sum, key range; 1: squared deviations + first select pass; 2-4: select (return at once when
+    // the median is already known).  Nothing is read back in between: the one-thread kernel steers the next pass.
+    for (int pass = 0; pass < 5; ++pass) {
+        rc = sweep_volume(v, st, grid,
+            [&](const float *p, unsigned long long n, int g) { launch_stat_pass_flat(pass, p, n, S, g, st); },
+            [&](const BoxK &box, int g) { launch_stat_pass_box(pass, box, S, g, st); });
+        if (rc != VR_OK) return rc;
+        launch_stat_step(S, pass, st);
+        v->stats.kernel_launches += 1;
+    }
+    if (out_location == VR_DEVICE) launch_stat_finish(S, out, st);
+    else {
+        launch_stat_finish(S, v->d_stat_out, st);
+        VR_CUDA(cudaMemcpyAsync(out, v->d_stat_out, sizeof(vr_statistics_result), cudaMemcpyDeviceToHost, st));
+        v->stats.d2h_bytes += sizeof(vr_statistics_result);
     }
     v->stats.kernel_launches += 1;
     VR_CUDA(cudaGetLastError());

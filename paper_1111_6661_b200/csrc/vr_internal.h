@@ -76,6 +76,25 @@ void launch_minmax_hist_flat(const float *v, unsigned long long n, uint32_t nbin
 void launch_minmax_hist_box(BoxK b, uint32_t nbins, SummaryScratch *s, int grid, cudaStream_t st);
 void launch_summary_finish(const SummaryScratch *s, uint32_t nbins, vr_summary *out, cudaStream_t st);
 
+// ---------------------------------------------------------------- mean / stddev / median (vr_stats.cu)
+constexpr int kStatMaxGrid = 1024;            // CTAs per pass launch (one double slot per CTA)
+struct StatScratch {
+    unsigned int klo, khi;                    // key interval that holds the median (pass 0: key of min / max)
+    unsigned int shift, done;                 // bin width 2^shift keys of the next select pass; 1: klo is the median
+    unsigned long long n_finite, n_nonfinite, rank;
+    double mean, m2, stddev;
+    unsigned long long hist[256];
+    unsigned long long part_n[kStatMaxGrid];
+    double part[kStatMaxGrid], part_c[kStatMaxGrid];
+};
+
+void launch_stat_reset(StatScratch *s, cudaStream_t st);
+// pass 0: count, sum, key range; 1: squared deviations + select; 2..4: select
+void launch_stat_pass_flat(int pass, const float *v, unsigned long long n, StatScratch *s, int grid, cudaStream_t st);
+void launch_stat_pass_box(int pass, BoxK b, StatScratch *s, int grid, cudaStream_t st);
+void launch_stat_step(StatScratch *s, int pass, cudaStream_t st);       // one thread, after pass `pass`
+void launch_stat_finish(const StatScratch *s, vr_statistics_result *out, cudaStream_t st);
+
 // ---------------------------------------------------------------- ray casting (vr_raycast.cu)
 struct TfK { const float4 *table; float scale, bias; };   // 257 float4 entries in global memory
 

@@ -15,35 +15,14 @@
 #include <float.h>
 
 #include "vr_internal.h"
+#include "vr_sweep.cuh"
 
 namespace vr {
 
 namespace {
 
-constexpr int kThreads = 512;
+constexpr int kThreads = kSweepThreads;
 constexpr int kHistSmemWords = 8192;          // 32 KB of uint32 counters
-
-__device__ __forceinline__ unsigned int enc_f(float f)
-{
-    const unsigned int b = __float_as_uint(f);
-    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
-}
-__device__ __forceinline__ float dec_f(unsigned int u)
-{
-    return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
-}
-
-__device__ __forceinline__ float4 ld_stream4(const float4 *p)
-{
-#ifdef VR_SIMT_HOST
-    return *p;
-#else
-    float4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
-                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
-    return r;
-#endif
-}
 
 struct Acc {                                   // per-thread running state
     float mn, mx;
@@ -150,28 +129,7 @@ k_reduce_flat(const float *__restrict__ v, unsigned long long n, uint32_t nbins,
     VR_DYN_SHARED(unsigned int, smem);
     const HistCtx hc = hist_begin<HIST>(s, nbins, smem);
     Acc a = { CUDART_INF_F, -CUDART_INF_F, 0u, 0u, 0u };
-    const unsigned long long n4 = n >> 2;
-    const float4 *v4 = reinterpret_cast<const float4 *>(v);
-    const unsigned long long stride = (unsigned long long)gridDim.x * kThreads;
-    unsigned long long i = (unsigned long long)blockIdx.x * kThreads + threadIdx.x;
-    for (; i + 3 * stride < n4; i += 4 * stride) {
-        const float4 x0 = ld_stream4(v4 + i), x1 = ld_stream4(v4 + i + stride);
-        const float4 x2 = ld_stream4(v4 + i + 2 * stride), x3 = ld_stream4(v4 + i + 3 * stride);
-        visit<MINMAX, HIST>(x0.x, a, hc); visit<MINMAX, HIST>(x0.y, a, hc);
-        visit<MINMAX, HIST>(x0.z, a, hc); visit<MINMAX, HIST>(x0.w, a, hc);
-        visit<MINMAX, HIST>(x1.x, a, hc); visit<MINMAX, HIST>(x1.y, a, hc);
-        visit<MINMAX, HIST>(x1.z, a, hc); visit<MINMAX, HIST>(x1.w, a, hc);
-        visit<MINMAX, HIST>(x2.x, a, hc); visit<MINMAX, HIST>(x2.y, a, hc);
-        visit<MINMAX, HIST>(x2.z, a, hc); visit<MINMAX, HIST>(x2.w, a, hc);
-        visit<MINMAX, HIST>(x3.x, a, hc); visit<MINMAX, HIST>(x3.y, a, hc);
-        visit<MINMAX, HIST>(x3.z, a, hc); visit<MINMAX, HIST>(x3.w, a, hc);
-    }
-    for (; i < n4; i += stride) {
-        const float4 x = ld_stream4(v4 + i);
-        visit<MINMAX, HIST>(x.x, a, hc); visit<MINMAX, HIST>(x.y, a, hc);
-        visit<MINMAX, HIST>(x.z, a, hc); visit<MINMAX, HIST>(x.w, a, hc);
-    }
-    if (blockIdx.x == 0 && threadIdx.x < (unsigned)(n & 3)) visit<MINMAX, HIST>(v[(n4 << 2) + threadIdx.x], a, hc);
+    sweep_flat(v, n, [&](float x) { visit<MINMAX, HIST>(x, a, hc); });
     finish_block<MINMAX, HIST>(a, hc, s);
 }
 
@@ -183,13 +141,7 @@ k_reduce_box(BoxK b, uint32_t nbins, SummaryScratch *s)
     VR_DYN_SHARED(unsigned int, smem);
     const HistCtx hc = hist_begin<HIST>(s, nbins, smem);
     Acc a = { CUDART_INF_F, -CUDART_INF_F, 0u, 0u, 0u };
-    const int lane = threadIdx.x & 31;
-    const long long rows = (long long)b.ey * b.ez;
-    const long long wstride = (long long)gridDim.x * (kThreads / 32);
-    for (long long r = (long long)blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5); r < rows; r += wstride) {
-        const float *row = b.base + (r % b.ey) * b.sy + (r / b.ey) * b.sz;
-        for (int x = lane; x < b.ex; x += 32) visit<MINMAX, HIST>(__ldg(row + x), a, hc);
-    }
+    sweep_box(b, [&](float x) { visit<MINMAX, HIST>(x, a, hc); });
     finish_block<MINMAX, HIST>(a, hc, s);
 }
 

@@ -102,6 +102,13 @@ def summary(be, vol, nbins=256, range_=None, device=True):
     return np.frombuffer(np.ascontiguousarray(raw).tobytes()[: 32 + 8 * nbins], dtype=vr.summary_dtype(nbins))[0]
 
 
+def statistics(be, vol, device=True):
+    buf = be.empty((40,), np.uint8, device=device)
+    vol.statistics(out=buf, stream=be.stream)
+    raw = be.numpy(buf)
+    return np.frombuffer(np.ascontiguousarray(raw).tobytes()[:40], dtype=vr.STATISTICS_DTYPE)[0]
+
+
 BACKENDS = {"gpu": GpuBackend(), "simt": SimtBackend()}
 BACKEND_PARAMS = [pytest.param("gpu", marks=pytest.mark.gpu), pytest.param("simt")]
 

@@ -45,9 +45,10 @@ def test_library_is_built_for_sm_100a_only():
 
 def test_struct_sizes_match_header(tmp_path):
     src = tmp_path / "sz.c"
-    src.write_text('#include "vr.h"\n#include <stdio.h>\n#include <stddef.h>\nint main(){printf("%zu %zu %zu %zu %zu %zu\\n",'
+    src.write_text('#include "vr.h"\n#include <stdio.h>\n#include <stddef.h>\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu %zu\\n",'
                    "sizeof(vr_volume_desc),sizeof(vr_camera),sizeof(vr_image),sizeof(vr_stats),"
-                   "offsetof(vr_summary,counts),offsetof(vr_volume_desc,data));return 0;}\n")
+                   "offsetof(vr_summary,counts),offsetof(vr_volume_desc,data),sizeof(vr_statistics_result),"
+                   "offsetof(vr_statistics_result,median));return 0;}\n")
     exe = tmp_path / "sz"
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
     got = [int(x) for x in subprocess.run([str(exe)], capture_output=True, text=True).stdout.split()]
@@ -57,6 +58,8 @@ def test_struct_sizes_match_header(tmp_path):
     assert got[3] == C.sizeof(binding.vr_stats)
     assert got[4] == 32 and binding.summary_dtype(256).itemsize == 32 + 8 * 256
     assert got[5] == binding.vr_volume_desc.data.offset
+    assert got[6] == C.sizeof(binding.vr_statistics_result) == binding.STATISTICS_DTYPE.itemsize == 40
+    assert got[7] == binding.vr_statistics_result.median.offset == 32
 
 
 def test_argument_errors_without_gpu():

@@ -10,7 +10,7 @@ import pytest
 import oracle as O
 import paper_1111_6661_b200 as vr
 import workload as W
-from backends import BACKENDS, be, render, summary  # noqa: F401  (be is a fixture)
+from backends import BACKENDS, be, render, statistics, summary  # noqa: F401  (be is a fixture)
 from parity import FRAGILE_FRAC_OPAQUE, check_ea, check_mip
 
 
@@ -48,6 +48,85 @@ def test_minmax_hist_nonfinite_and_constant(be):
     with vr.Volume(be.dev(k), (32, 16, 8)) as vol:
         g = summary(be, vol)
         assert np.all(g["counts"] == k.size // 256)
+
+
+# ------------------------------------------------------------------ §8(f) #1: mean, standard deviation, median
+def assert_statistics_equal(g, o, v):
+    """Counts and the median (a data value) bit-exact; the float64 moments within 1e-13 of the data scale: both
+    sides sum in compensated float64, in different orders (S35-S36)."""
+    assert int(g["n_finite"]) == o.n_finite and int(g["n_nonfinite"]) == o.n_nonfinite
+    if o.n_finite == 0:
+        assert np.isnan(g["mean"]) and np.isnan(g["stddev"]) and np.isnan(g["median"])
+        return
+    assert np.float32(g["median"]).tobytes() == np.float32(o.median).tobytes(), (g["median"], o.median)
+    f = v[np.isfinite(v)].astype(np.float64)
+    scale = np.abs(f).mean()
+    assert abs(float(g["mean"]) - o.mean) <= 1e-13 * scale, (g["mean"], o.mean)
+    assert abs(float(g["stddev"]) - o.stddev) <= 1e-13 * max(o.stddev, scale), (g["stddev"], o.stddev)
+
+
+@pytest.mark.parametrize("dims", [(128, 128, 128), (37, 29, 41), (130, 67, 3), (2, 2, 2)])
+def test_statistics_match_oracle(be, dims):
+    nx, ny, nz = dims
+    if not be.full and nx * ny * nz > 200000:
+        nx, ny, nz = 96, 50, 40
+    v = W.make_cube(W.Recipe(nx, ny, nz, seed=23, n_sources=4 if nx > 8 else 0)).copy()
+    if v.size > 100:
+        v.reshape(-1)[[3, 50, 97]] = np.nan, np.inf, -np.inf
+    with vr.Volume(be.dev(v), (nx, ny, nz)) as vol:
+        g = statistics(be, vol)
+        assert_statistics_equal(g, O.statistics(v), v)
+        g2 = statistics(be, vol, device=False)                       # pinned host output, and run-to-run determinism
+        assert g.tobytes() == g2.tobytes()
+
+
+def test_statistics_special_cubes(be):
+    """Constant cube (the key interval is a single key after pass 0), a two-valued cube with even n (LOWER median),
+    signed zeros (totalOrder: -0 before +0), integers 0..255 (closed forms), no finite voxel at all."""
+    cases = []
+    cases.append(np.full((5, 6, 7), -3.25, dtype=np.float32))
+    two = np.array([1.0] * 30 + [5.0] * 30, dtype=np.float32).reshape(3, 4, 5)
+    cases.append(two)
+    two2 = two.copy(); two2[0, 0, 0] = 5.0
+    cases.append(two2)
+    z = np.array([0.0, -0.0, -0.0, 0.0, 1.0, -1.0, -0.0, 2.0], dtype=np.float32).reshape(2, 2, 2)
+    cases.append(z)
+    z2 = z.copy(); z2[0, 0, 1] = 0.0
+    cases.append(z2)
+    k = np.repeat(np.arange(256), 32).astype(np.float32)
+    np.random.default_rng(4).shuffle(k)
+    cases.append(k.reshape(8, 32, 32))
+    cases.append(np.full((3, 4, 5), np.nan, dtype=np.float32))
+    wide = np.array([-3.0e38, 3.0e38, 1e-45, -1e-45, 0.5, 7.0, -2.0, 1.0], dtype=np.float32).reshape(2, 2, 2)   # the whole key space
+    cases.append(wide)
+    for c in cases:
+        nz, ny, nx = c.shape
+        with vr.Volume(be.dev(c), (nx, ny, nz)) as vol:
+            g = statistics(be, vol)
+        o = O.statistics(c)
+        assert_statistics_equal(g, o, c)
+        if np.isfinite(c).all():
+            assert np.float32(g["median"]).tobytes() == np.sort(c.reshape(-1))[(c.size - 1) // 2].tobytes() or \
+                float(g["median"]) == 0.0                             # np.sort does not order the signed zeros
+    with vr.Volume(be.dev(cases[5]), (32, 32, 8)) as vol:
+        g = statistics(be, vol)
+    assert g["mean"] == 127.5 and g["median"] == 127.0 and abs(g["stddev"] - np.sqrt((256 ** 2 - 1) / 12)) < 1e-12
+
+
+@pytest.mark.parametrize("where", ["device", "host_ooc"])
+def test_statistics_bricked_halo_and_streamed(be, where):
+    """Halo voxels are not counted; out of core all five passes ride the brick streamer."""
+    n, B = (45, 38, 52), 16
+    v = W.make_cube(W.Recipe(*n, seed=36, n_sources=4)).copy()
+    v[7, 8, 9] = np.nan
+    t = W.retile_halo(v, B)
+    kw = dict(resident_bytes=7 * (B + 1) ** 3 * 4, n_copy_streams=3) if where == "host_ooc" else {}
+    data = be.dev(t) if where == "device" else be.pinned(t)
+    with vr.Volume(data, n, brick=B, layout=vr.VR_BRICKED_HALO1, **kw) as vol:
+        g = statistics(be, vol)
+        assert_statistics_equal(g, O.statistics(v), v)
+        if where == "host_ooc":
+            assert vol.stats()["h2d_bytes"] > 4 * t.size              # the non-resident bricks were streamed five times
 
 
 # ------------------------------------------------------------------ cfg1: A3, A6-A9
@@ -389,6 +468,28 @@ def _lattice(cfg, stride=8):
     return m
 
 
+def _check_statistics_by_definition(g, v):
+    """At sizes the oracle's sort cannot finish in seconds: the properties that DEFINE the results.  The median m is
+    a voxel value with #(v < m) <= rank < #(v <= m), rank = (n-1)//2; mean and stddev against float64 slab sums."""
+    n = v.size
+    assert int(g["n_finite"]) == n and int(g["n_nonfinite"]) == 0
+    m = np.float32(g["median"])
+    below = le = 0
+    s1 = 0.0
+    slabs = np.array_split(np.arange(v.shape[0]), max(1, v.nbytes >> 28))
+    for idx in slabs:
+        blk = v[idx[0]:idx[-1] + 1]
+        below += int(np.count_nonzero(blk < m)); le += int(np.count_nonzero(blk <= m))
+        s1 += float(blk.sum(dtype=np.float64))
+    assert below <= (n - 1) // 2 < le, (below, le, n)
+    mean = s1 / n
+    s2 = 0.0
+    for idx in slabs:
+        d = v[idx[0]:idx[-1] + 1].astype(np.float64) - mean
+        s2 += float(np.dot(d.reshape(-1), d.reshape(-1)))
+    assert abs(float(g["mean"]) - mean) <= 1e-11 and abs(float(g["stddev"]) - np.sqrt(s2 / n)) <= 1e-11
+
+
 def _full_size_case(number, views, summary_exact=True, stride=8):
     """vr_minmax_histogram on the whole cube (bit-exact) and vr_render of `views` at the config's own image
     size, step, ERT and flags — the launches bench.py times — compared with the oracle on a lattice of every
@@ -407,6 +508,7 @@ def _full_size_case(number, views, summary_exact=True, stride=8):
             assert_summary_equal(g, O.minmax_hist(v))
         vmin, vmax = float(g["vmin"]), float(g["vmax"])
         R = max(abs(vmin), abs(vmax))
+        _check_statistics_by_definition(statistics(b, vol), v)
         vol.set_transfer_function(tf, vmin, vmax)
         for view in views:
             cam = cfg.camera(view)
