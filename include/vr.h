@@ -109,8 +109,11 @@ VR_API vr_status vr_destroy_volume(vr_volume *vol);
  *   vmin,vmax  scalar range mapped to u in [0,1]: scale = 1/(vmax-vmin), bias = -vmin*scale,
  *          both rounded to float32 once (C.4).  Must be finite with vmax > vmin.  Normally
  *          the vmin/vmax produced by vr_minmax_histogram.
- * The table is uploaded with a synchronous copy; safe to call between frames.
- * Errors: VR_ERR_INVALID_ARG, VR_ERR_CUDA.
+ * Host work only: the table reaches the device on the stream of the next vr_render that needs it, so renders
+ * already enqueued keep the table they were launched with.  A handle is used on ONE stream at a time: calls
+ * on different streams must be ordered by the caller (event or synchronisation), because the handle's device
+ * table, summary scratch and staging buffers are single instances.
+ * Errors: VR_ERR_INVALID_ARG.
  * ------------------------------------------------------------------------------------------ */
 VR_API vr_status vr_set_transfer_function(vr_volume *vol, const float *rgba, float vmin, float vmax);
 
@@ -240,7 +243,10 @@ typedef struct {
     uint64_t total_kernel_launches; /* since vr_create_volume */
     uint64_t resident_bytes;        /* device bytes owned by the handle */
     uint32_t zfast_copy;            /* 1: the handle holds a z-fastest copy of the volume (VR_OPT_ZFAST_COPY) */
-    uint32_t reserved;
+    uint32_t skip_variant;          /* 1: the last render launched the empty-space-skipping kernel variant */
+    uint64_t macro_cells;           /* macrocells of the skipping grid (0: none built) */
+    uint64_t empty_cells;           /* cells whose samples all have opacity 0 under the current transfer function,
+                                       as of the last flag pass that has COMPLETED on its stream */
 } vr_stats;
 
 VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
@@ -258,9 +264,16 @@ VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
  *                       array, slower).  The voxel data must not change while a handle holds a copy.
  *   VR_OPT_LANE_LAG     lane-mapped path: a ray more than this many voxel planes (along the view's principal
  *                       axis) ahead of the slowest ray of its warp waits; 0 = off; default 1.
+ *   VR_OPT_EMPTY_SKIP   1 (default): exact transfer-function-aware empty-space skipping on the lane-mapped path
+ *                       (SURVEY.md §8(f) #2).  When the table has an interval of opacity exactly 0, the library
+ *                       keeps min / max per macrocell of 8^3 voxels (one extra read of the volume, once per
+ *                       handle) and one byte per cell and transfer function; a sample based in a cell whose
+ *                       whole value range maps to opacity 0 is not read (compositing it would change nothing,
+ *                       C.5), so images are bit-identical.  Used only while at least 1/64 of the cells are
+ *                       empty (decided on the device, no read-back).  0: never.
  * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).
  * ------------------------------------------------------------------------------------------ */
-enum { VR_OPT_RENDER_PATH = 1, VR_OPT_ZFAST_COPY = 2, VR_OPT_LANE_LAG = 3 };
+enum { VR_OPT_RENDER_PATH = 1, VR_OPT_ZFAST_COPY = 2, VR_OPT_LANE_LAG = 3, VR_OPT_EMPTY_SKIP = 4 };
 VR_API vr_status vr_set_option(vr_volume *vol, uint32_t option, int64_t value);
 
 /* Thread-local message of the last failing call on this thread ("" if none). */

@@ -18,7 +18,7 @@ VR_LINEAR, VR_BRICKED_HALO1 = 0, 1
 VR_DEVICE, VR_HOST_PINNED = 0, 1
 VR_EA, VR_MIP = 0, 1
 VR_SORT_LAST = 1
-VR_OPT_RENDER_PATH, VR_OPT_ZFAST_COPY, VR_OPT_LANE_LAG = 1, 2, 3
+VR_OPT_RENDER_PATH, VR_OPT_ZFAST_COPY, VR_OPT_LANE_LAG, VR_OPT_EMPTY_SKIP = 1, 2, 3, 4
 VR_PATH_AUTO, VR_PATH_RAY_MAJOR = 0, 1
 
 _STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_UNSUPPORTED", 3: "VR_ERR_OUT_OF_MEMORY",
@@ -54,7 +54,8 @@ class vr_stats(C.Structure):
                 ("bricks_culled", C.c_uint32), ("path", C.c_uint32), ("kernel_launches", C.c_uint32),
                 ("fragments", C.c_uint64), ("h2d_bytes", C.c_uint64), ("d2h_bytes", C.c_uint64),
                 ("total_kernel_launches", C.c_uint64), ("resident_bytes", C.c_uint64),
-                ("zfast_copy", C.c_uint32), ("reserved", C.c_uint32)]
+                ("zfast_copy", C.c_uint32), ("skip_variant", C.c_uint32), ("macro_cells", C.c_uint64),
+                ("empty_cells", C.c_uint64)]
 
 
 class vr_statistics_result(C.Structure):

@@ -89,10 +89,19 @@ struct vr_volume {
     cudaStream_t copy[kMaxCopyStreams] = {};
     int n_copy = 0;
 
-    // transfer function
+    // transfer function: host copy; uploaded on the stream of the next render that needs it
     float4 *d_tf = nullptr;
-    bool tf_set = false;
+    float tf_tab[257 * 4];
+    bool tf_set = false, tf_dirty = false, tf_has_zero = false;
     float tf_scale = 0.0f, tf_bias = 0.0f;
+
+    // exact empty-space skipping (vr_macro.cu): macrocell min/max (made once), per-transfer-function flags
+    float2 *macro_mm = nullptr;
+    unsigned char *macro_flag = nullptr;
+    unsigned long long *d_nskip = nullptr, *h_nskip = nullptr;
+    bool macro_failed = false, macro_flags_dirty = true;
+    int mc[3] = { 0, 0, 0 };
+    int opt_skip = 1;
 
     // scratch
     SummaryScratch *d_sum = nullptr;
@@ -135,6 +144,10 @@ static void free_volume(vr_volume *v)
     if (v->d_stat) cudaFree(v->d_stat);
     if (v->d_stat_out) cudaFree(v->d_stat_out);
     if (v->zfast) cudaFree(v->zfast);
+    if (v->macro_mm) cudaFree(v->macro_mm);
+    if (v->macro_flag) cudaFree(v->macro_flag);
+    if (v->d_nskip) cudaFree(v->d_nskip);
+    if (v->h_nskip) cudaFreeHost(v->h_nskip);
     if (v->zfast_ev) cudaEventDestroy(v->zfast_ev);
     v->arena.release();
     v->host_image.release();
@@ -437,10 +450,75 @@ static vr_status ensure_zfast(vr_volume *v, cudaStream_t st, bool *have)
     return VR_OK;
 }
 
+// The table set by vr_set_transfer_function reaches the device on the stream of the first render that uses it
+// (stream order: renders already enqueued on that stream keep the table they were launched with).
+static vr_status upload_tf(vr_volume *v, cudaStream_t st)
+{
+    if (!v->tf_dirty) return VR_OK;
+    Staging *s;
+    vr_status rc = staging_acquire(v, sizeof(v->tf_tab), &s);
+    if (rc != VR_OK) return rc;
+    memcpy(s->h, v->tf_tab, sizeof(v->tf_tab));
+    VR_CUDA(cudaMemcpyAsync(v->d_tf, s->h, sizeof(v->tf_tab), cudaMemcpyHostToDevice, st));
+    VR_CUDA(cudaEventRecord(s->done, st));
+    s->in_flight = true;
+    v->stats.h2d_bytes += sizeof(v->tf_tab);
+    v->tf_dirty = false;
+    return VR_OK;
+}
+
+// Macrocell grid of a resident linear volume (made once, on the render's stream) and the per-transfer-function
+// flags (remade after every vr_set_transfer_function).  Leaves M.flag == nullptr when skipping cannot be used.
+static vr_status ensure_macro(vr_volume *v, const TfK &tf, cudaStream_t st, MacroK &M)
+{
+    M.flag = nullptr; M.n_skip = nullptr; M.min_skip = ~0ull; M.cx = M.cy = M.cz = 0;
+    v->stats.skip_variant = 0;
+    if (!v->opt_skip || !v->tf_has_zero || v->macro_failed || v->desc.layout != VR_LINEAR || v->out_of_core) return VR_OK;
+    const int n[3] = { (int)v->desc.nx, (int)v->desc.ny, (int)v->desc.nz };
+    if (!v->macro_mm) {
+        for (int a = 0; a < 3; ++a) v->mc[a] = (n[a] - 2) / kMacroEdge + 1;       // base indices 0 .. n-2
+        const size_t cells = (size_t)v->mc[0] * v->mc[1] * v->mc[2];
+        if (v->mc[2] > 65535 || cells > 0x7fffffffull) { v->macro_failed = true; return VR_OK; }
+        float2 *mm = nullptr; unsigned char *fl = nullptr;
+        if (cudaMalloc(&mm, cells * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); v->macro_failed = true; return VR_OK; }
+        if (cudaMalloc(&fl, cells) != cudaSuccess) { cudaGetLastError(); cudaFree(mm); v->macro_failed = true; return VR_OK; }
+        v->macro_mm = mm; v->macro_flag = fl;
+        VR_CUDA(cudaMalloc(&v->d_nskip, sizeof(unsigned long long)));
+        VR_CUDA(cudaMallocHost(&v->h_nskip, sizeof(unsigned long long)));
+        *v->h_nskip = 0;
+        MacroK G; G.flag = nullptr; G.n_skip = nullptr; G.min_skip = 0; G.cx = v->mc[0]; G.cy = v->mc[1]; G.cz = v->mc[2];
+        launch_macro_minmax(v->dev_data, n[0], n[1], n[2], G, v->macro_mm, st);
+        v->stats.kernel_launches += 1;
+        v->stats.resident_bytes += cells * (sizeof(float2) + 1);
+        v->macro_flags_dirty = true;
+    }
+    const long long cells = (long long)v->mc[0] * v->mc[1] * v->mc[2];
+    if (v->macro_flags_dirty) {
+        VR_CUDA(cudaMemsetAsync(v->d_nskip, 0, sizeof(unsigned long long), st));
+        launch_macro_flags(v->macro_mm, cells, tf, v->macro_flag, v->d_nskip,
+                           (int)std::min<long long>((cells + 255) / 256, (long long)v->sm_count * 8), st);
+        VR_CUDA(cudaMemcpyAsync(v->h_nskip, v->d_nskip, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        MacroK G; G.flag = nullptr; G.n_skip = nullptr; G.min_skip = 0; G.cx = v->mc[0]; G.cy = v->mc[1]; G.cz = v->mc[2];
+        launch_macro_blocks(v->macro_flag, G, (int)std::min<long long>((cells / 512 + 8) / 8, (long long)v->sm_count * 8), st);
+        v->stats.kernel_launches += 2;
+        v->macro_flags_dirty = false;
+    }
+    M.flag = v->macro_flag; M.n_skip = v->d_nskip;
+    M.min_skip = (unsigned long long)std::max<long long>(1, cells / 64);      // worth a byte load per sample from ~1.6 % empty cells
+    M.cx = v->mc[0]; M.cy = v->mc[1]; M.cz = v->mc[2];
+    v->stats.skip_variant = 1;
+    v->stats.macro_cells = (uint64_t)cells;
+    return VR_OK;
+}
+
 static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, const TfK &tf,
                               float *img, long long pitch_f, cudaStream_t st)
 {
     const int n[3] = { (int)v->desc.nx, (int)v->desc.ny, (int)v->desc.nz };
+    MacroK Mc;
+    Mc.flag = nullptr; Mc.n_skip = nullptr; Mc.min_skip = ~0ull; Mc.cx = Mc.cy = Mc.cz = 0;
+    if (mode == VR_EA) { vr_status rc = ensure_macro(v, tf, st, Mc); if (rc != VR_OK) return rc; }
+    else v->stats.skip_variant = 0;
     // how many of 9 probe pixels (corners, edge midpoints, centre) travel mostly along x
     int n_x = 0;
     for (int py = 0; py < 3; ++py)
@@ -459,17 +537,17 @@ static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam,
     int rows;
     if (!have_z || n_x == 0) {
         make_lane_map(c, n, 0, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else if (n_x == 9) {
         make_lane_map(c, n, 2, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else {
         make_lane_map(c, n, 0, 1, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, rows, img, pitch_f, st);
         make_lane_map(c, n, 2, 2, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, rows, img, pitch_f, st);
         v->stats.kernel_launches += 2;
     }
     v->stats.path = 7;
@@ -622,16 +700,17 @@ VR_API vr_status vr_set_transfer_function(vr_volume *v, const float *rgba, float
     g_err[0] = 0;
     VR_REQUIRE(v && rgba, "vr_set_transfer_function: NULL argument");
     VR_REQUIRE(std::isfinite(vmin) && std::isfinite(vmax) && vmax > vmin, "need finite vmin < vmax (got %g, %g)", vmin, vmax);
-    float tab[257 * 4];
-    for (int i = 0; i < 1024; ++i) {
+    bool has_zero = false;
+    for (int i = 0; i < 1024; ++i)
         VR_REQUIRE(std::isfinite(rgba[i]) && rgba[i] >= 0.0f && rgba[i] <= 1.0f, "table entry %d = %g is outside [0,1]", i, rgba[i]);
-        tab[i] = rgba[i];
-    }
-    for (int c = 0; c < 4; ++c) tab[1024 + c] = rgba[1020 + c];      // pad entry (never weighted: i <= 254)
-    VR_CUDA(cudaSetDevice(v->device));
-    VR_CUDA(cudaMemcpy(v->d_tf, tab, sizeof(tab), cudaMemcpyHostToDevice));
+    for (int i = 0; i < 1024; ++i) v->tf_tab[i] = rgba[i];
+    for (int c = 0; c < 4; ++c) v->tf_tab[1024 + c] = rgba[1020 + c];      // pad entry (never weighted: i <= 254)
+    for (int i = 0; i < 255; ++i) has_zero = has_zero || (rgba[4 * i + 3] == 0.0f && rgba[4 * i + 7] == 0.0f);
+    v->tf_has_zero = has_zero;                                       // some table interval has opacity exactly 0
     v->tf_scale = 1.0f / (vmax - vmin);                             // C.4, float32
     v->tf_bias = -vmin * v->tf_scale;
+    v->tf_dirty = true;                                             // uploaded on the stream of the next render
+    v->macro_flags_dirty = true;
     v->tf_set = true;
     return VR_OK;
 }
@@ -684,6 +763,7 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     vr_status rc = ensure_mirror(v, st);
     if (rc != VR_OK) return rc;
 
+    if (mode == VR_EA) { rc = upload_tf(v, st); if (rc != VR_OK) return rc; }
     const CamK cam = to_camk(c);
     TfK tf; tf.table = v->d_tf; tf.scale = v->tf_scale; tf.bias = v->tf_bias;
     if (sort_last) rc = render_sort_last(v, c, cam, mode, tf, img, pitch_f, st);
@@ -808,6 +888,9 @@ VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
     case VR_OPT_LANE_LAG:
         VR_REQUIRE(value >= 0 && value <= 1024, "VR_OPT_LANE_LAG: 0..1024 base planes (got %lld)", (long long)value);
         v->opt_lag = (int)value; return VR_OK;
+    case VR_OPT_EMPTY_SKIP:
+        VR_REQUIRE(value == 0 || value == 1, "VR_OPT_EMPTY_SKIP: 0 never, 1 when the transfer function has empty intervals (got %lld)", (long long)value);
+        v->opt_skip = (int)value; return VR_OK;
     default:
         set_error("unknown option %u", option); return VR_ERR_INVALID_ARG;
     }
@@ -819,6 +902,7 @@ VR_API vr_status vr_get_stats(vr_volume *v, vr_stats *s)
     VR_REQUIRE(v && s, "vr_get_stats: NULL argument");
     VR_REQUIRE(s->struct_size == sizeof(vr_stats), "vr_stats.struct_size %u != %zu", s->struct_size, sizeof(vr_stats));
     *s = v->stats;
+    s->empty_cells = v->h_nskip ? (uint64_t)*v->h_nskip : 0;          // as of the last completed flag pass
     return VR_OK;
 }
 

@@ -40,6 +40,14 @@ inline void vr_launch(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, 
 #endif
 }
 
+// event counters for the host emulation of the tests (nothing in the product build)
+#ifdef VR_SIMT_HOST
+#define VR_TEST_COUNT(i) (++::simt::g_counters[i])
+#else
+#define VR_TEST_COUNT(i) ((void)0)
+#endif
+enum { VR_CNT_LEAP_CELL = 0, VR_CNT_LEAP_BLOCK = 1, VR_CNT_LEAP_REJECTED = 2, VR_CNT_LAG_WAIT = 3 };
+
 // dynamic shared memory of the CTA as an array of T
 #ifdef VR_SIMT_HOST
 #define VR_DYN_SHARED(T, name) T *name = reinterpret_cast<T *>(::simt::g_dyn_smem)
@@ -133,8 +141,24 @@ struct LaneVolK {
     int nx, ny, nz;
 };
 
+// exact empty-space skipping (vr_macro.cu): one byte per macrocell of kMacroEdge^3 base indices; bit 0 = every
+// sample based in the cell has opacity exactly 0 under the current transfer function, bit 1 = so has every cell
+// of its block of 8 x 8 x 8 cells; n_skip = how many cells have bit 0 set
+constexpr int kMacroEdge = 8;
+struct MacroK {
+    const unsigned char *flag;                // nullptr: no skipping
+    const unsigned long long *n_skip;         // device counter written by the flag kernel
+    unsigned long long min_skip;              // skipping is used iff *n_skip >= min_skip (decided on the device)
+    int cx, cy, cz;                           // cells per axis
+};
+
+void launch_macro_minmax(const float *v, int nx, int ny, int nz, const MacroK &m, float2 *mm, cudaStream_t st);
+void launch_macro_flags(const float2 *mm, long long n_cells, const TfK &tf, unsigned char *flag, unsigned long long *n_skip,
+                        int grid, cudaStream_t st);
+void launch_macro_blocks(unsigned char *flag, const MacroK &m, int grid, cudaStream_t st);
+
 void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
-                 int rows, float *image, long long pitch_f, cudaStream_t st);
+                 const MacroK &macro, int rows, float *image, long long pitch_f, cudaStream_t st);
 void launch_transpose_xz(const float *in, float *out, int nx, int ny, int nz, cudaStream_t st);
 
 }  // namespace vr

@@ -85,12 +85,48 @@ __device__ __forceinline__ float sample_cell(const LaneVolK &V, int ix, int iy, 
         return trilerp_packed(q00, q10, r00, r10, q01, q11, r01, r11, fx, fy, fz);
 }
 
-template <int MODE, bool ERT, bool WIDE, int FAST>
+// Empty-space leap (vr_macro.cu): sample k of the ray, at parameter t with base index (ix,iy,iz), lies in an empty
+// cell of 2^lg base indices per axis.  Returns n >= 1 such that samples k .. k+n-1 all lie in that cell (so all
+// have opacity exactly 0 and may be skipped).  n is ESTIMATED from the slab exit of the cell and then VERIFIED:
+// base indices are monotone in t on every axis, so if the position of sample k+n-1 (or the ray's exit point, if
+// that comes first) has the same cell, every sample in between has it too; otherwise n = 1.  The march continues from the canonical t_{k+n} = fma(k+n, step, t_first).
+__device__ __forceinline__ float leap_samples(int lg, const Ray &r, const float *inv, float inv_step, float step, float t,
+                                              float kf, int ix, int iy, int iz, int nx, int ny, int nz)
+{
+    const int i[3] = { ix, iy, iz };
+    float t_out = CUDART_INF_F;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int org = (i[a] >> lg) << lg;
+        const float bound = (float)(r.d[a] > 0.0f ? org + (1 << lg) : org);
+        if (r.d[a] != 0.0f) t_out = fminf(t_out, (bound - r.oc[a]) * inv[a]);
+    }
+    float nf = fminf(fmaxf(floorf((t_out - t) * inv_step), 1.0f), 65536.0f);      // NaN -> 1
+    if (nf > 1.0f) {
+        // the last skipped sample, or the exit point of the ray when that comes first (the cell of a position is
+        // monotone in t for every real t, so the samples up to the exit are covered as well)
+        const float tl = fminf(__fmaf_rn(__fadd_rn(kf, __fsub_rn(nf, 1.0f)), step, r.t_first), r.t_exit);
+        int jx, jy, jz;
+        float g;
+        axis_cell(tl, r.d[0], r.oc[0], nx, jx, g);
+        axis_cell(tl, r.d[1], r.oc[1], ny, jy, g);
+        axis_cell(tl, r.d[2], r.oc[2], nz, jz, g);
+        const bool same = (jx >> lg) == (ix >> lg) && (jy >> lg) == (iy >> lg) && (jz >> lg) == (iz >> lg);
+        if (!same) { nf = 1.0f; VR_TEST_COUNT(VR_CNT_LEAP_REJECTED); }
+        else VR_TEST_COUNT(lg == 6 ? VR_CNT_LEAP_BLOCK : VR_CNT_LEAP_CELL);
+    }
+    return nf;
+}
+
+template <int MODE, bool ERT, bool WIDE, int FAST, bool SKIP>
 __global__ void __launch_bounds__(kLaneThreads)
-k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, float *__restrict__ image, long long pitch_f)
+k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, float *__restrict__ image, long long pitch_f)
 {
     __shared__ TfS tf_s;
     if (MODE == VR_EA) stage_tf_pairs(tf_s, tf);
+    // exact empty-space skipping (vr_macro.cu): used only when enough cells are empty under this transfer function
+    const bool skipping = SKIP && __ldg(Mc.n_skip) >= Mc.min_skip;
+    const int cxy = Mc.cx * Mc.cy;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // pixel of this lane: p along the lane axis, q = sheared row + off(p)
     const int p = blockIdx.x * 32 + lane;
@@ -111,6 +147,12 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, float *__restrict__ image, long
     float cr = 0.0f, cg = 0.0f, cb = 0.0f, T = 1.0f, m = -CUDART_INF_F;
     float kf = 0.0f;
     const int lag = M.lag;
+    float inv[3] = { 0.0f, 0.0f, 0.0f };
+    const float inv_step = SKIP ? 1.0f / cam.step : 0.0f;
+    if (SKIP) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) inv[a] = 1.0f / r.d[a];          // only used by the leap estimate (d_a != 0 checked there)
+    }
     for (;;) {
         const float t = __fmaf_rn(kf, cam.step, r.t_first);
         alive = alive && t < r.t_exit;                               // C.2: sample k exists iff t_k < t_exit
@@ -126,15 +168,22 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, float *__restrict__ image, long
             const int prog = M.psign >= 0 ? ip : -ip;
             const int slowest = __reduce_min_sync(0xffffffffu, alive ? prog : INT_MAX);
             go = alive && prog - slowest <= lag;
+            if (alive && !go) VR_TEST_COUNT(VR_CNT_LAG_WAIT);
         }
         if (go) {
-            const float s = sample_cell<WIDE, FAST>(V, ix, iy, iz, fx, fy, fz);
-            if (MODE == VR_MIP) m = fmaxf(m, s);
-            else {
-                composite_p(classify_s(tf_s, tf.scale, tf.bias, s), cr, cg, cb, T);
-                if (ERT && T <= cam.t_min) alive = false;           // stop AFTER compositing this sample (C.5)
-            }
-            kf = __fadd_rn(kf, 1.0f);                                // exact: k < 2^24
+            // a sample based in an empty macrocell has opacity exactly 0: compositing it changes nothing (C.5)
+            unsigned int empty = 0u;
+            if (SKIP && skipping) empty = __ldg(Mc.flag + ((iz >> 3) * cxy + (iy >> 3) * Mc.cx + (ix >> 3)));
+            if (!SKIP || empty == 0u) {
+                const float s = sample_cell<WIDE, FAST>(V, ix, iy, iz, fx, fy, fz);
+                if (MODE == VR_MIP) m = fmaxf(m, s);
+                else {
+                    composite_p(classify_s(tf_s, tf.scale, tf.bias, s), cr, cg, cb, T);
+                    if (ERT && T <= cam.t_min) alive = false;       // stop AFTER compositing this sample (C.5)
+                }
+                kf = __fadd_rn(kf, 1.0f);                            // exact: k < 2^24
+            } else                                                   // leap to the end of the empty cell (or block of cells)
+                kf = __fadd_rn(kf, leap_samples((empty & 2u) ? 6 : 3, r, inv, inv_step, cam.step, t, kf, ix, iy, iz, V.nx, V.ny, V.nz));
         }
     }
     if (!mine) return;
@@ -165,7 +214,7 @@ k_transpose_xz(const float *__restrict__ in, float *__restrict__ out, int nx, in
 }  // namespace
 
 void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
-                 int rows, float *image, long long pitch_f, cudaStream_t st)
+                 const MacroK &macro, int rows, float *image, long long pitch_f, cudaStream_t st)
 {
     const int P = map.lane_axis == 0 ? cam.width : cam.height;
     const dim3 g((unsigned)((P + 31) / 32), (unsigned)((rows + kRowsPerCta - 1) / kRowsPerCta));
@@ -174,7 +223,9 @@ void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int f
                                     (unsigned long long)((fast == 0 ? vol.ny : vol.nx) - 1) * (unsigned long long)vol.sa +
                                     (unsigned long long)(fast == 0 ? vol.nx : vol.nz);
     const bool wide = span > 0xffffffffull;
-#define VR_L3(M, E, Wd, F) vr_launch(k_rows<M, E, Wd, F>, g, kLaneThreads, 0, st, cam, vol, tf, map, image, pitch_f)
+    const bool skip = mode == VR_EA && macro.flag != nullptr;
+#define VR_L4(M, E, Wd, F, S) vr_launch(k_rows<M, E, Wd, F, S>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, image, pitch_f)
+#define VR_L3(M, E, Wd, F) do { if (M == VR_EA && skip) VR_L4(M, E, Wd, F, (M == VR_EA)); else VR_L4(M, E, Wd, F, false); } while (0)
 #define VR_L2(M, E, Wd) do { if (fast == 0) VR_L3(M, E, Wd, 0); else VR_L3(M, E, Wd, 2); } while (0)
 #define VR_L1(M, E) do { if (wide) VR_L2(M, E, true); else VR_L2(M, E, false); } while (0)
     if (mode == VR_MIP) VR_L1(VR_MIP, false);
@@ -183,6 +234,7 @@ void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int f
 #undef VR_L1
 #undef VR_L2
 #undef VR_L3
+#undef VR_L4
 }
 
 void launch_transpose_xz(const float *in, float *out, int nx, int ny, int nz, cudaStream_t st)

@@ -105,6 +105,7 @@ namespace simt {
 struct Builtins { uint3 tid, bid; dim3 bdim, gdim; };
 extern Builtins g_cur;                     // built-in variables of the running fiber
 extern unsigned char *g_dyn_smem;          // dynamic shared memory of the running CTA
+extern unsigned long long g_counters[16];  // VR_TEST_COUNT(i) of vr_internal.h
 
 struct KernelBody { void (*fn)(void *); void *ctx; };
 void launch_cta_grid(dim3 grid, dim3 block, size_t dyn_smem, KernelBody body);

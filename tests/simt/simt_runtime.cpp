@@ -33,6 +33,7 @@ namespace simt {
 
 Builtins g_cur;
 unsigned char *g_dyn_smem = nullptr;
+unsigned long long g_counters[16] = {};
 
 namespace {
 
@@ -304,6 +305,9 @@ __attribute__((visibility("default"))) void *simt_device_alloc(size_t n) { retur
 __attribute__((visibility("default"))) void *simt_pinned_alloc(size_t n) { return guarded_alloc(n ? n : 1, 1); }
 __attribute__((visibility("default"))) void simt_free(void *p) { guarded_free(p); }
 __attribute__((visibility("default"))) size_t simt_device_bytes_in_use(void) { return g_device_bytes; }
+// event counters the kernels bump through VR_TEST_COUNT (vr_internal.h): tests assert that a code path really ran
+__attribute__((visibility("default"))) unsigned long long simt_counter(int i) { return i >= 0 && i < 16 ? simt::g_counters[i] : 0; }
+__attribute__((visibility("default"))) void simt_reset_counters(void) { for (auto &c : simt::g_counters) c = 0; }
 __attribute__((visibility("default"))) void simt_set_device_capacity(size_t n) { g_device_capacity = n; }
 
 cudaError_t cudaMalloc(void **p, size_t n)

@@ -255,6 +255,94 @@ def test_lane_mapped_views(be, n, variant):
         assert vol.stats()["zfast_copy"] == variant[1]            # the x-travelling views made the copy (when allowed)
 
 
+# ------------------------------------------------------------------ §8(f) #2: exact empty-space skipping
+@pytest.mark.parametrize("n", [(132, 72, 100), (61, 47, 83)])
+def test_empty_space_skipping_is_exact(be, n):
+    """TF_SOURCES makes the noise floor transparent (opacity exactly 0 on a table interval): most macrocells are
+    empty, the kernel skips their samples, and the image is STILL bit-identical to the oracle, which skips nothing
+    (C.5: compositing a sample of opacity 0 changes nothing).  Cells next to sources, cells with NaN / Inf voxels
+    and the clamped outer half voxel are the cases a wrong cell range would get wrong."""
+    if not be.full:
+        n = tuple(max(24, d // 2) for d in n)
+    v = W.make_cube(W.Recipe(*n, seed=93, n_sources=10 if be.full else 2)).copy()
+    v[n[2] // 2, n[1] // 2, n[0] // 3] = np.nan
+    v[3, 4, 5] = np.inf
+    s = O.minmax_hist(v)
+    tf = W.tf_sources(n, 0.5, alpha_scale=8.0)
+    views = [(k, c) for k, c in _axis_views(n, be.full) if k in ("persp0", "persp2", "persp5", "persp6", "ortho_x", "inside", "axis_x")]
+    with vr.Volume(be.dev(v), n) as vol:
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for name, cam in views:
+            for ert in (0.0, 0.99):
+                cam2 = cam.with_(ert_alpha=ert)
+                oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax)
+                g = render(be, vol, cam2, vr.VR_EA)
+                assert np.array_equal(g, oe.image, equal_nan=True), (name, ert)
+                st = vol.stats()
+                assert st["path"] == 7 and st["skip_variant"] == 1
+        st = vol.stats()
+        assert st["macro_cells"] == np.prod([(d - 2) // 8 + 1 for d in n])
+        assert st["empty_cells"] >= st["macro_cells"] // 4          # the skipping really happened
+        # a transfer function without an empty interval: the plain variant, same handle
+        tf2 = W.tf_opaque(n, 0.5).copy(); tf2[:, 3] = np.maximum(tf2[:, 3], 1e-3)
+        vol.set_transfer_function(tf2, s.vmin, s.vmax)
+        name, cam = views[0]
+        oe = O.render(v, cam, O.EA, tf2, s.vmin, s.vmax)
+        assert np.array_equal(render(be, vol, cam, vr.VR_EA), oe.image, equal_nan=True)
+        assert vol.stats()["skip_variant"] == 0
+        # TF_HAZE has an empty interval but no cell of a noise cube falls into it: the variant is launched and
+        # decides on the device not to skip
+        tf3 = W.tf_haze(n, 0.5)
+        vol.set_transfer_function(tf3, s.vmin, s.vmax)
+        oe = O.render(v, cam, O.EA, tf3, s.vmin, s.vmax)
+        assert np.array_equal(render(be, vol, cam, vr.VR_EA), oe.image, equal_nan=True)
+        be.sync()
+        assert vol.stats()["skip_variant"] == 1 and vol.stats()["empty_cells"] < max(1, vol.stats()["macro_cells"] // 64)
+        vol.set_option(vr.VR_OPT_EMPTY_SKIP, 0)
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
+        assert np.array_equal(render(be, vol, cam, vr.VR_EA), oe.image, equal_nan=True)
+        assert vol.stats()["skip_variant"] == 0
+
+
+def test_empty_space_leaps_over_whole_blocks(be):
+    """A cube that is empty (under the transfer function) except for one corner: blocks of 8x8x8 cells are empty as
+    a whole and rays leap 64 base indices at a time; rays that graze the blob, enter through the clamped outer half
+    voxel or end inside an empty block exercise the verification of every leap."""
+    n = (150, 80, 90) if be.full else (136, 72, 72)
+    nx, ny, nz = n
+    rng = np.random.default_rng(17)
+    v = (-1.0 + 0.05 * rng.standard_normal((nz, ny, nx))).astype(np.float32)
+    z, y, x = np.mgrid[0:nz, 0:ny, 0:nx]
+    v += (12.0 * np.exp(-((x - 20.0) ** 2 + (y - 15.0) ** 2 + (z - 18.0) ** 2) / (2 * 6.0 ** 2))).astype(np.float32)
+    v[nz - 1, ny - 1, nx - 1] = 9.0                                  # one bright voxel in the far corner
+    s = O.minmax_hist(v)
+    tf = W.tf_sources(n, 0.5, alpha_scale=6.0)
+    c = np.array(n, dtype=np.float64) / 2
+    m = float(max(n))
+    size = (64, 40) if be.full else (40, 26)
+    cams = [W.perspective_camera(c + np.array(e) * m, c, (0, 1, 0), 40.0, *size, step=st)
+            for e, st in (((1.7, 0.3, 0.2), 0.5), ((-0.4, 0.5, 1.6), 1.0), ((-1.2, -0.9, -1.1), 0.25))]
+    cams.append(W.ortho_axis_camera(n, 0, +1, step=1.0, width=size[0], height=size[1]))
+    if be.name == "simt":
+        import simt_lib
+        simt_lib.lib().simt_reset_counters()
+    with vr.Volume(be.dev(v), n) as vol:
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for cam in cams:
+            for ert in (0.0, 0.99):
+                cam2 = cam.with_(ert_alpha=ert)
+                oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax)
+                assert np.array_equal(render(be, vol, cam2, vr.VR_EA), oe.image), ert
+                assert oe.image[..., 3].max() > 0.05                 # the blob is visible: not everything was skipped
+        st = vol.stats()
+        assert st["skip_variant"] == 1 and st["empty_cells"] > 0.8 * st["macro_cells"]
+    if be.name == "simt":                                           # the emulation counts what the kernel did
+        cnt = [simt_lib.lib().simt_counter(i) for i in range(4)]
+        assert cnt[0] > 1000 and cnt[1] > 1000, cnt                  # leaps over single cells AND over whole blocks
+        assert cnt[2] < 0.2 * (cnt[0] + cnt[1]), cnt                 # the estimate is rarely rejected by the verification
+
+
 def test_zfast_copy_skipped_when_memory_is_short(be):
     """Without room for a second copy of the volume the x-travelling views render from the x-fastest array."""
     if be.name != "simt":
@@ -398,7 +486,7 @@ def test_host_linear_mirror_and_host_outputs(be):
         oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
         check_ea(g, oe.image, oe.fragile, oe.K > 0)
         assert vol.stats()["d2h_bytes"] == g.size * 4
-        assert vol.stats()["h2d_bytes"] < 4096                           # per-frame tables only; the cube is not re-uploaded
+        assert vol.stats()["h2d_bytes"] <= 257 * 16                      # the transfer function only; the cube is not re-uploaded
 
 
 def test_pageable_host_memory_is_rejected(be):

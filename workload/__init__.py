@@ -11,12 +11,12 @@ from .cubes import (Recipe, CubeGenerator, make_cube, checksum, retile_halo, bri
                     build as build_generator)
 from .cameras import (Camera, ortho_axis_camera, perspective_camera, orbit_camera, ortho_lookat_camera,
                       nominal_samples)
-from .transfer import TF_HAZE_POINTS, bake_tf, tf_haze, tf_opaque
+from .transfer import TF_HAZE_POINTS, TF_SOURCES_POINTS, bake_tf, tf_haze, tf_opaque, tf_sources
 from .configs import CONFIGS, WorkloadConfig, get_config
 
 __all__ = [
     "Recipe", "CubeGenerator", "make_cube", "checksum", "retile_halo", "bricked_halo_elems", "fill_bricked_halo_ptr", "build_generator",
     "Camera", "ortho_axis_camera", "perspective_camera", "orbit_camera", "ortho_lookat_camera", "nominal_samples",
-    "TF_HAZE_POINTS", "bake_tf", "tf_haze", "tf_opaque",
+    "TF_HAZE_POINTS", "TF_SOURCES_POINTS", "bake_tf", "tf_haze", "tf_opaque", "tf_sources",
     "CONFIGS", "WorkloadConfig", "get_config",
 ]

@@ -40,3 +40,20 @@ def tf_haze(dims, step: float) -> np.ndarray:
 def tf_opaque(dims, step: float) -> np.ndarray:
     """TF_OPAQUE: TF_HAZE with alpha x25 clamped to 1 (ERT parity workload; ERT-assisted timing)."""
     return bake_tf(TF_HAZE_POINTS, step, alpha_scale=25.0 * kappa(dims))
+
+
+# sources only: everything below u = 0.40 (about +5 sigma of the noise on the configs' cubes, whose range is
+# roughly [-5, 21] .. [-10, 27]) is fully transparent
+TF_SOURCES_POINTS = (
+    (0.00, 0.0, 0.0, 0.0, 0.0),
+    (0.40, 0.0, 0.1, 0.4, 0.0),
+    (0.50, 0.1, 0.5, 0.9, 0.05),
+    (0.70, 0.9, 0.8, 0.2, 0.3),
+    (1.00, 1.0, 1.0, 1.0, 0.8),
+)
+
+
+def tf_sources(dims, step: float, alpha_scale: float = 1.0) -> np.ndarray:
+    """TF_SOURCES: the noise floor is transparent (opacity exactly 0 on a table interval), the compact sources are
+    emissive — what an astronomer sets to look at detections; the workload of exact empty-space skipping."""
+    return bake_tf(TF_SOURCES_POINTS, step, alpha_scale=alpha_scale * kappa(dims))
