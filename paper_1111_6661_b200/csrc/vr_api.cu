@@ -313,6 +313,13 @@ static vr_status render_single(vr_volume *v, const CamK &cam, int mode, bool ert
     return VR_OK;
 }
 
+static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, const TfK &tf,
+                              const PartK *part, float *img, long long pitch_f, cudaStream_t st);
+
+// Sort-last (C.7, A10): per-(pixel, brick) fragments over each brick's screen rectangle, folded per pixel in
+// visibility order by k_composite.  Fragments of a VR_LINEAR volume come from ONE lane-mapped march per frame
+// that flushes the ray state at every change of owner brick; bricks of a resident VR_BRICKED_HALO1 volume are
+// marched one (brick, pixel tile) per CTA.  Both produce the same fragments bit for bit.
 static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, const TfK &tf,
                                   float *img, long long pitch_f, cudaStream_t st)
 {
@@ -338,9 +345,12 @@ static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &
     for (size_t i = 0; i < bin_cnt.size(); ++i) { const uint32_t c2 = bin_cnt[i]; bin_cnt[i] = (uint32_t)n_list; n_list += c2; }
     if (n_work > 0x7fffffffull) { set_error("too many (brick, tile) work items: %zu", n_work); return VR_ERR_UNSUPPORTED; }
 
+    const bool lanes = v->desc.layout == VR_LINEAR && v->opt_path == 0;
+    // the lane-mapped march needs no work items: a brick-grid -> plan-index table takes their place
+    const size_t work_bytes = lanes ? (size_t)v->n_bricks * sizeof(int) : n_work * sizeof(WorkK);
     const size_t off_bricks = 0;
     const size_t off_work = (off_bricks + plan.size() * sizeof(BrickK) + 255) & ~(size_t)255;
-    const size_t off_offs = (off_work + n_work * sizeof(WorkK) + 255) & ~(size_t)255;
+    const size_t off_offs = (off_work + work_bytes + 255) & ~(size_t)255;
     const size_t off_list = (off_offs + bin_cnt.size() * sizeof(uint32_t) + 255) & ~(size_t)255;
     const size_t total = off_list + n_list * sizeof(uint32_t) + 256;
     Staging *s;
@@ -356,12 +366,17 @@ static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &
         const BrickK &k = plan[bi].k;
         hb[bi] = k;
         const int tw = (k.x1 - k.x0 + 15) / 16, th = (k.y1 - k.y0 + 7) / 8;
-        for (int ty = 0; ty < th; ++ty)
+        for (int ty = 0; ty < th && !lanes; ++ty)
             for (int tx = 0; tx < tw; ++tx) { hw[wi].brick = (int)bi; hw[wi].tx = tx; hw[wi].ty = ty; hw[wi].pad = 0; ++wi; }
         for (int ty = k.y0 / 16; ty <= (k.y1 - 1) / 16; ++ty)
             for (int tx = k.x0 / 16; tx <= (k.x1 - 1) / 16; ++tx) hl[fill[(size_t)ty * bins_x + tx]++] = (uint32_t)bi;
     }
     memcpy(ho, bin_cnt.data(), bin_cnt.size() * sizeof(uint32_t));
+    if (lanes) {
+        int *lut = reinterpret_cast<int *>(hw);
+        for (uint64_t b = 0; b < v->n_bricks; ++b) lut[b] = -1;
+        for (size_t bi = 0; bi < plan.size(); ++bi) lut[plan[bi].id] = (int)bi;
+    }
 
     rc = v->arena.reserve((size_t)n_frag * (mode == VR_EA ? 4 : 1) + 4);
     if (rc != VR_OK) return rc;
@@ -373,8 +388,20 @@ static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &
     Vdims.base = nullptr; Vdims.sy = Vdims.sz = 0; Vdims.ox = Vdims.oy = Vdims.oz = 0;
     // 64-bit element offsets only when a linear volume exceeds 2^32-1 voxels; slots never do
     const bool wide = v->desc.layout == VR_LINEAR && v->n_vox > 0xffffffffull;
-    launch_march_bricks(mode, wide, cam, Vdims, tf, reinterpret_cast<const BrickK *>(s->d + off_bricks),
-                        reinterpret_cast<const WorkK *>(s->d + off_work), (int)n_work, v->arena.p, st);
+    if (lanes) {
+        launch_fragment_init(mode, v->arena.p, n_frag, v->sm_count * 8, st);
+        PartK P;
+        P.bricks = reinterpret_cast<const BrickK *>(s->d + off_bricks);
+        P.lut = reinterpret_cast<const int *>(s->d + off_work);
+        P.arena = v->arena.p; P.B = (int)v->B; P.nbx = (int)v->nb[0]; P.nby = (int)v->nb[1];
+        if (n_frag) v->stats.kernel_launches += 1;
+        rc = render_lanes(v, c, cam, mode, false, tf, &P, img, pitch_f, st);      // counts its own one or two launches
+        if (rc != VR_OK) return rc;
+    } else {
+        launch_march_bricks(mode, wide, cam, Vdims, tf, reinterpret_cast<const BrickK *>(s->d + off_bricks),
+                            reinterpret_cast<const WorkK *>(s->d + off_work), (int)n_work, v->arena.p, st);
+        if (n_work) v->stats.kernel_launches += 1;
+    }
     BinsK bins;
     bins.offs = reinterpret_cast<const unsigned int *>(s->d + off_offs);
     bins.list = reinterpret_cast<const unsigned int *>(s->d + off_list);
@@ -382,7 +409,7 @@ static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &
     launch_composite(mode, cam, reinterpret_cast<const BrickK *>(s->d + off_bricks), bins, v->arena.p, img, pitch_f, st);
     VR_CUDA(cudaEventRecord(s->done, st));
     s->in_flight = true;
-    v->stats.kernel_launches += (n_work ? 1 : 0) + 1;
+    v->stats.kernel_launches += 1;
     v->stats.path = 2;
     v->stats.fragments = n_frag;
     v->stats.bricks_drawn = (uint32_t)plan.size();
@@ -511,13 +538,14 @@ static vr_status ensure_macro(vr_volume *v, const TfK &tf, cudaStream_t st, Macr
     return VR_OK;
 }
 
+// part != nullptr: per-(ray, owner brick) fragments for the sort-last compositor instead of pixels
 static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, const TfK &tf,
-                              float *img, long long pitch_f, cudaStream_t st)
+                              const PartK *part, float *img, long long pitch_f, cudaStream_t st)
 {
     const int n[3] = { (int)v->desc.nx, (int)v->desc.ny, (int)v->desc.nz };
     MacroK Mc;
     Mc.flag = nullptr; Mc.n_skip = nullptr; Mc.min_skip = ~0ull; Mc.cx = Mc.cy = Mc.cz = 0;
-    if (mode == VR_EA) { vr_status rc = ensure_macro(v, tf, st, Mc); if (rc != VR_OK) return rc; }
+    if (mode == VR_EA && !part) { vr_status rc = ensure_macro(v, tf, st, Mc); if (rc != VR_OK) return rc; }
     else v->stats.skip_variant = 0;
     // how many of 9 probe pixels (corners, edge midpoints, centre) travel mostly along x
     int n_x = 0;
@@ -537,17 +565,17 @@ static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam,
     int rows;
     if (!have_z || n_x == 0) {
         make_lane_map(c, n, 0, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else if (n_x == 9) {
         make_lane_map(c, n, 2, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else {
         make_lane_map(c, n, 0, 1, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, rows, img, pitch_f, st);
         make_lane_map(c, n, 2, 2, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, rows, img, pitch_f, st);
         v->stats.kernel_launches += 2;
     }
     v->stats.path = 7;
@@ -769,7 +797,7 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     if (sort_last) rc = render_sort_last(v, c, cam, mode, tf, img, pitch_f, st);
     else if (v->out_of_core || v->desc.layout == VR_BRICKED_HALO1) rc = render_chain(v, c, cam, mode, ert, tf, img, pitch_f, st);
     else if (v->opt_path == 1) rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
-    else rc = render_lanes(v, c, cam, mode, ert, tf, img, pitch_f, st);
+    else rc = render_lanes(v, c, cam, mode, ert, tf, nullptr, img, pitch_f, st);
     if (rc != VR_OK) return rc;
     VR_CUDA(cudaGetLastError());
     if (im->location == VR_HOST_PINNED) {

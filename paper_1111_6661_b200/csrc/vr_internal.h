@@ -157,8 +157,19 @@ void launch_macro_flags(const float2 *mm, long long n_cells, const TfK &tf, unsi
                         int grid, cudaStream_t st);
 void launch_macro_blocks(unsigned char *flag, const MacroK &m, int grid, cudaStream_t st);
 
+// sort-last partials written by the lane-mapped kernel: plan-ordered brick table, brick-grid -> plan index (-1:
+// culled), fragment arena, brick edge and grid
+struct PartK {
+    const BrickK *bricks;
+    const int *lut;
+    float *arena;
+    int B, nbx, nby;
+};
+
+// part != nullptr: write per-(ray, owner brick) fragments instead of pixels (no ERT, C.7)
 void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
-                 const MacroK &macro, int rows, float *image, long long pitch_f, cudaStream_t st);
+                 const MacroK &macro, const PartK *part, int rows, float *image, long long pitch_f, cudaStream_t st);
+void launch_fragment_init(int mode, float *arena, unsigned long long n_frag, int grid, cudaStream_t st);
 void launch_transpose_xz(const float *in, float *out, int nx, int ny, int nz, cudaStream_t st);
 
 }  // namespace vr

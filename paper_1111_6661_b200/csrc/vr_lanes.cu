@@ -118,9 +118,25 @@ __device__ __forceinline__ float leap_samples(int lg, const Ray &r, const float 
     return nf;
 }
 
-template <int MODE, bool ERT, bool WIDE, int FAST, bool SKIP>
+// sort-last partials (C.7): writes the fragment (C_b, T_b) / m_b of pixel (i,j) for the brick with plan index `cur`
+template <int MODE>
+__device__ __forceinline__ void flush_fragment(const PartK &P, int cur, int i, int j, float cr, float cg, float cb, float T,
+                                               float m)
+{
+    const BrickK *b = P.bricks + cur;
+    const int x0 = __ldg(&b->x0), y0 = __ldg(&b->y0), x1 = __ldg(&b->x1), y1 = __ldg(&b->y1);
+    if (i < x0 || i >= x1 || j < y0 || j >= y1) return;          // never: the screen rectangle holds every owning pixel (A4)
+    const unsigned long long f = __ldg(&b->frag_off) + (unsigned long long)(j - y0) * (unsigned)(x1 - x0) + (unsigned)(i - x0);
+    if (MODE == VR_MIP) P.arena[f] = m;
+    else reinterpret_cast<float4 *>(P.arena)[f] = make_float4(cr, cg, cb, T);
+}
+
+// PART: instead of one pixel value per ray, one fragment per (ray, owner brick): the ray state is flushed to the
+// brick's fragment and reset whenever the owner brick (ix/B, iy/B, iz/B) of the next sample changes — the same
+// samples in the same order as the per-brick marches of C.7, so the fragments are bit-identical to theirs.
+template <int MODE, bool ERT, bool WIDE, int FAST, bool SKIP, bool PART>
 __global__ void __launch_bounds__(kLaneThreads)
-k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, float *__restrict__ image, long long pitch_f)
+k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__restrict__ image, long long pitch_f)
 {
     __shared__ TfS tf_s;
     if (MODE == VR_EA) stage_tf_pairs(tf_s, tf);
@@ -147,6 +163,7 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, float *__restrict__ 
     float cr = 0.0f, cg = 0.0f, cb = 0.0f, T = 1.0f, m = -CUDART_INF_F;
     float kf = 0.0f;
     const int lag = M.lag;
+    int cur = -1, blo[3] = { 1, 1, 1 }, bhi[3] = { 0, 0, 0 };      // PART: plan index and base-index box of the owner brick
     float inv[3] = { 0.0f, 0.0f, 0.0f };
     const float inv_step = SKIP ? 1.0f / cam.step : 0.0f;
     if (SKIP) {
@@ -170,6 +187,14 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, float *__restrict__ 
             go = alive && prog - slowest <= lag;
             if (alive && !go) VR_TEST_COUNT(VR_CNT_LAG_WAIT);
         }
+        if (PART && go && (ix < blo[0] || ix > bhi[0] || iy < blo[1] || iy > bhi[1] || iz < blo[2] || iz > bhi[2])) {
+            if (cur >= 0) flush_fragment<MODE>(P, cur, i, j, cr, cg, cb, T, m);
+            const int bx = ix / P.B, by = iy / P.B, bz = iz / P.B;
+            cur = __ldg(P.lut + (bz * P.nby + by) * P.nbx + bx);
+            blo[0] = bx * P.B; blo[1] = by * P.B; blo[2] = bz * P.B;
+            bhi[0] = blo[0] + P.B - 1; bhi[1] = blo[1] + P.B - 1; bhi[2] = blo[2] + P.B - 1;
+            cr = cg = cb = 0.0f; T = 1.0f; m = -CUDART_INF_F;
+        }
         if (go) {
             // a sample based in an empty macrocell has opacity exactly 0: compositing it changes nothing (C.5)
             unsigned int empty = 0u;
@@ -187,10 +212,25 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, float *__restrict__ 
         }
     }
     if (!mine) return;
+    if (PART) {
+        if (cur >= 0) flush_fragment<MODE>(P, cur, i, j, cr, cg, cb, T, m);
+        return;
+    }
     if (MODE == VR_MIP) image[(long long)j * pitch_f + i] = m;
     else
         *reinterpret_cast<float4 *>(image + (long long)j * pitch_f + 4 * (long long)i) =
             make_float4(cr, cg, cb, __fsub_rn(1.0f, T));
+}
+
+// identity fragments (C.7): a pixel of a brick's rectangle whose ray owns no sample in the brick folds as nothing
+template <int MODE>
+__global__ void __launch_bounds__(256) k_fragment_init(float *__restrict__ arena, unsigned long long n_frag)
+{
+    const unsigned long long stride = (unsigned long long)gridDim.x * 256;
+    for (unsigned long long f = (unsigned long long)blockIdx.x * 256 + threadIdx.x; f < n_frag; f += stride) {
+        if (MODE == VR_MIP) arena[f] = -CUDART_INF_F;
+        else reinterpret_cast<float4 *>(arena)[f] = make_float4(0.0f, 0.0f, 0.0f, 1.0f);
+    }
 }
 
 // z-fastest copy: out[x][y][z] = in[z][y][x]; one CTA transposes a 32 (x) by 32 (z) tile of one y
@@ -214,18 +254,23 @@ k_transpose_xz(const float *__restrict__ in, float *__restrict__ out, int nx, in
 }  // namespace
 
 void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
-                 const MacroK &macro, int rows, float *image, long long pitch_f, cudaStream_t st)
+                 const MacroK &macro, const PartK *part, int rows, float *image, long long pitch_f, cudaStream_t st)
 {
-    const int P = map.lane_axis == 0 ? cam.width : cam.height;
-    const dim3 g((unsigned)((P + 31) / 32), (unsigned)((rows + kRowsPerCta - 1) / kRowsPerCta));
+    const int n_lane = map.lane_axis == 0 ? cam.width : cam.height;
+    const dim3 g((unsigned)((n_lane + 31) / 32), (unsigned)((rows + kRowsPerCta - 1) / kRowsPerCta));
     if (g.x == 0 || g.y == 0) return;
     const unsigned long long span = (unsigned long long)((fast == 0 ? vol.nz : vol.ny) - 1) * (unsigned long long)vol.sb +
                                     (unsigned long long)((fast == 0 ? vol.ny : vol.nx) - 1) * (unsigned long long)vol.sa +
                                     (unsigned long long)(fast == 0 ? vol.nx : vol.nz);
     const bool wide = span > 0xffffffffull;
-    const bool skip = mode == VR_EA && macro.flag != nullptr;
-#define VR_L4(M, E, Wd, F, S) vr_launch(k_rows<M, E, Wd, F, S>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, image, pitch_f)
-#define VR_L3(M, E, Wd, F) do { if (M == VR_EA && skip) VR_L4(M, E, Wd, F, (M == VR_EA)); else VR_L4(M, E, Wd, F, false); } while (0)
+    const bool skip = mode == VR_EA && macro.flag != nullptr && !part;
+    PartK P;
+    if (part) P = *part;
+    else { P.bricks = nullptr; P.lut = nullptr; P.arena = nullptr; P.B = 1; P.nbx = P.nby = 0; }
+#define VR_L4(M, E, Wd, F, S) vr_launch(k_rows<M, E, Wd, F, S, false>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f)
+#define VR_L3(M, E, Wd, F) do { \
+        if (part) vr_launch(k_rows<M, false, Wd, F, false, true>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f); \
+        else if (M == VR_EA && skip) VR_L4(M, E, Wd, F, (M == VR_EA)); else VR_L4(M, E, Wd, F, false); } while (0)
 #define VR_L2(M, E, Wd) do { if (fast == 0) VR_L3(M, E, Wd, 0); else VR_L3(M, E, Wd, 2); } while (0)
 #define VR_L1(M, E) do { if (wide) VR_L2(M, E, true); else VR_L2(M, E, false); } while (0)
     if (mode == VR_MIP) VR_L1(VR_MIP, false);
@@ -235,6 +280,13 @@ void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int f
 #undef VR_L2
 #undef VR_L3
 #undef VR_L4
+}
+
+void launch_fragment_init(int mode, float *arena, unsigned long long n_frag, int grid, cudaStream_t st)
+{
+    if (n_frag == 0) return;
+    if (mode == VR_MIP) vr_launch(k_fragment_init<VR_MIP>, grid, 256, 0, st, arena, n_frag);
+    else vr_launch(k_fragment_init<VR_EA>, grid, 256, 0, st, arena, n_frag);
 }
 
 void launch_transpose_xz(const float *in, float *out, int nx, int ny, int nz, cudaStream_t st)

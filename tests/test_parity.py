@@ -394,14 +394,20 @@ def test_all_miss_camera(be):
 
 
 # ------------------------------------------------------------------ bricks: A0, A4, A10
-@pytest.mark.parametrize("B", [7, 16, 32, 100])
-def test_sort_last_equals_oracle_bricked(be, B):
+@pytest.mark.parametrize("B,how", [(7, "lanes"), (16, "lanes"), (32, "lanes"), (100, "lanes"), (16, "tiles"), (16, "halo")])
+def test_sort_last_equals_oracle_bricked(be, B, how):
+    """Fragments from the lane-mapped march that flushes at every change of owner brick (`lanes`, the default for
+    linear volumes), from one CTA per (brick, pixel tile) on a linear volume (`tiles`) and on a resident brick-major
+    volume with halo (`halo`): all bit-identical to the oracle's bricked render (same partials, same fold order)."""
     n = (61, 47, 83)
     v = W.make_cube(W.Recipe(*n, seed=33, n_sources=5))
     s = O.minmax_hist(v)
     R = float(max(abs(s.vmin), abs(s.vmax)))
     tf = W.bake_tf(W.TF_HAZE_POINTS, 0.5, alpha_scale=6.0)
-    with vr.Volume(be.dev(v), n, brick=B) as vol:
+    data = be.dev(W.retile_halo(v, B)) if how == "halo" else be.dev(v)
+    with vr.Volume(data, n, brick=B, layout=vr.VR_BRICKED_HALO1 if how == "halo" else vr.VR_LINEAR) as vol:
+        if how == "tiles":
+            vol.set_option(vr.VR_OPT_RENDER_PATH, vr.VR_PATH_RAY_MAJOR)
         vol.set_transfer_function(tf, s.vmin, s.vmax)
         for name, cam in _views(n):
             cam = cam.with_(flags=W.cameras.VR_SORT_LAST)
