@@ -653,6 +653,46 @@ def test_cfg4_full_size_sampled():
     _full_size_case(4, views=(5, 12), summary_exact=True, stride=16)
 
 
+@pytest.mark.gpu
+def test_cfg5_scaled_out_of_core():
+    """cfg5 at 1/8 linear scale: 512x512x384 brick-major (+1 halo) in pinned host memory as 32^3 bricks — the SAME
+    16x16x12 = 3072-brick grid as cfg5 —, 25 % of the cube resident, 4 copy streams, 8 orbit views 480x270, step 0.5,
+    EA + ERT 0.99, plus the streamed min/max + histogram and statistics.  Renders on the every-4th-pixel lattice and the
+    summary are bit-identical to the oracle reading the same brick-major bytes."""
+    import torch
+    from dataclasses import replace
+    b = BACKENDS["gpu"]
+    cfg = W.get_config(5)
+    n, B = (512, 512, 384), 32
+    rec = replace(cfg.recipe, nx=n[0], ny=n[1], nz=n[2], n_sources=40)
+    n_el = W.bricked_halo_elems(n, B)
+    host = torch.empty(n_el, dtype=torch.float32, pin_memory=True)
+    W.fill_bricked_halo_ptr(rec, B, host.data_ptr())
+    hn = host.numpy().reshape(-1, B + 1, B + 1, B + 1)
+    o_sum = O.minmax_hist(hn, layout=O.BRICKED_HALO1, layout_brick=B, dims=n)
+    tf = W.tf_haze(n, 0.5)
+    Wd, H = 480, 270
+    mask = np.zeros((H, Wd), dtype=np.uint8)
+    mask[2::4, 2::4] = 1
+    sel = mask.astype(bool)
+    with vr.Volume(host, n, brick=B, layout=vr.VR_BRICKED_HALO1, resident_bytes=n_el * 4 // 4, n_copy_streams=4) as vol:
+        assert_summary_equal(summary(b, vol, device=False), o_sum)
+        h2d_summary = vol.stats()["h2d_bytes"]
+        assert h2d_summary >= n_el * 4                                # pass 1 streams everything, pass 2 the non-resident rest
+        g = statistics(b, vol)
+        assert int(g["n_finite"]) == n[0] * n[1] * n[2]
+        vol.set_transfer_function(tf, float(o_sum.vmin), float(o_sum.vmax))
+        for view in range(8):
+            cam = W.orbit_camera(n, view, 8, Wd, H, step=0.5, ert_alpha=0.99)
+            o = O.render(hn, cam, O.EA, tf, o_sum.vmin, o_sum.vmax, mask=mask, layout=O.BRICKED_HALO1, layout_brick=B, dims=n)
+            gi = render(b, vol, cam, vr.VR_EA)
+            st = vol.stats()
+            assert st["path"] == 3 and st["h2d_bytes"] >= 0.7 * n_el * 4 and st["bricks_drawn"] + st["bricks_culled"] == 3072
+            s = check_ea(gi[sel], o.image[sel], o.fragile[sel], (o.K > 0)[sel])
+            assert s["bit_exact"] == 1.0, (view, s)
+    del host
+
+
 # ------------------------------------------------------------------ S24: non-finite voxels in a rendered cube
 def test_nonfinite_voxels_render_like_the_oracle(be):
     """FITS blanks: NaN and +-Inf voxels.  A NaN sample classifies as table entry 0 and is ignored by MIP (C.4, C.6,
