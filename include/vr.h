@@ -271,9 +271,11 @@ VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
  *                       whole value range maps to opacity 0 is not read (compositing it would change nothing,
  *                       C.5), so images are bit-identical.  Used only while at least 1/64 of the cells are
  *                       empty (decided on the device, no read-back).  0: never.
+ *   VR_OPT_FORCE_WIDE   1: the render kernels form 64-bit voxel offsets even for volumes of fewer than 2^32
+ *                       voxels (the code the largest volumes run; lets the tests cover it at small size).  Default 0.
  * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).
  * ------------------------------------------------------------------------------------------ */
-enum { VR_OPT_RENDER_PATH = 1, VR_OPT_ZFAST_COPY = 2, VR_OPT_LANE_LAG = 3, VR_OPT_EMPTY_SKIP = 4 };
+enum { VR_OPT_RENDER_PATH = 1, VR_OPT_ZFAST_COPY = 2, VR_OPT_LANE_LAG = 3, VR_OPT_EMPTY_SKIP = 4, VR_OPT_FORCE_WIDE = 5 };
 VR_API vr_status vr_set_option(vr_volume *vol, uint32_t option, int64_t value);
 
 /* Thread-local message of the last failing call on this thread ("" if none). */

@@ -114,7 +114,7 @@ struct vr_volume {
     float *zfast = nullptr;
     bool zfast_failed = false;                // allocation refused once: not retried
     cudaEvent_t zfast_ev = nullptr;           // recorded after the transposition
-    int opt_path = 0, opt_zcopy = 1, opt_lag = 1;   // vr_set_option
+    int opt_path = 0, opt_zcopy = 1, opt_lag = 1, opt_wide = 0;   // vr_set_option
     Staging staging[kStagingRing];
     int staging_next = 0;
 
@@ -306,7 +306,7 @@ static vr_status render_single(vr_volume *v, const CamK &cam, int mode, bool ert
     VolK V;
     V.base = v->dev_data; V.sy = v->desc.nx; V.sz = (long long)v->desc.nx * v->desc.ny;
     V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz; V.ox = V.oy = V.oz = 0;
-    launch_march_full(mode, ert, cam, V, tf, img, pitch_f, st);
+    launch_march_full(mode, ert, v->opt_wide != 0, cam, V, tf, img, pitch_f, st);
     v->stats.kernel_launches += 1;
     v->stats.path = 1;
     v->stats.bricks_drawn = (uint32_t)v->n_bricks;
@@ -315,6 +315,7 @@ static vr_status render_single(vr_volume *v, const CamK &cam, int mode, bool ert
 
 static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, const TfK &tf,
                               const PartK *part, float *img, long long pitch_f, cudaStream_t st);
+static bool lanes_addressable(const vr_volume *v);
 
 // Sort-last (C.7, A10): per-(pixel, brick) fragments over each brick's screen rectangle, folded per pixel in
 // visibility order by k_composite.  Fragments of a VR_LINEAR volume come from ONE lane-mapped march per frame
@@ -345,7 +346,7 @@ static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &
     for (size_t i = 0; i < bin_cnt.size(); ++i) { const uint32_t c2 = bin_cnt[i]; bin_cnt[i] = (uint32_t)n_list; n_list += c2; }
     if (n_work > 0x7fffffffull) { set_error("too many (brick, tile) work items: %zu", n_work); return VR_ERR_UNSUPPORTED; }
 
-    const bool lanes = v->desc.layout == VR_LINEAR && v->opt_path == 0;
+    const bool lanes = v->desc.layout == VR_LINEAR && v->opt_path == 0 && lanes_addressable(v);
     // the lane-mapped march needs no work items: a brick-grid -> plan-index table takes their place
     const size_t work_bytes = lanes ? (size_t)v->n_bricks * sizeof(int) : n_work * sizeof(WorkK);
     const size_t off_bricks = 0;
@@ -387,7 +388,7 @@ static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &
     Vdims.nx = (int)v->desc.nx; Vdims.ny = (int)v->desc.ny; Vdims.nz = (int)v->desc.nz;
     Vdims.base = nullptr; Vdims.sy = Vdims.sz = 0; Vdims.ox = Vdims.oy = Vdims.oz = 0;
     // 64-bit element offsets only when a linear volume exceeds 2^32-1 voxels; slots never do
-    const bool wide = v->desc.layout == VR_LINEAR && v->n_vox > 0xffffffffull;
+    const bool wide = v->opt_wide != 0 || (v->desc.layout == VR_LINEAR && v->n_vox > 0xffffffffull);
     if (lanes) {
         launch_fragment_init(mode, v->arena.p, n_frag, v->sm_count * 8, st);
         PartK P;
@@ -439,7 +440,7 @@ static vr_status render_chain(vr_volume *v, const vr_camera *c, const CamK &cam,
             p.k.base = ptr; p.k.sy = v->E; p.k.sz = (long long)v->E * v->E;
             p.k.ox = (int)(p.b[0] * v->B); p.k.oy = (int)(p.b[1] * v->B); p.k.oz = (int)(p.b[2] * v->B);
         } else resident_brick_view(v, p.b[0], p.b[1], p.b[2], p.k);
-        launch_chain_brick(mode, ert, cam, V, tf, p.k, img, pitch_f, st);
+        launch_chain_brick(mode, ert, v->opt_wide != 0, cam, V, tf, p.k, img, pitch_f, st);
         v->stats.kernel_launches += 1;
         if (v->out_of_core) { vr_status rc = stream_brick_release(v, slot, st); if (rc != VR_OK) return rc; }
     }
@@ -538,6 +539,12 @@ static vr_status ensure_macro(vr_volume *v, const TfK &tf, cudaStream_t st, Macr
     return VR_OK;
 }
 
+// the lane-mapped kernel forms offsets inside one plane of either volume copy in 32 bits
+static bool lanes_addressable(const vr_volume *v)
+{
+    return (uint64_t)v->desc.nx * v->desc.ny <= 0xffffffffull && (uint64_t)v->desc.ny * v->desc.nz <= 0xffffffffull;
+}
+
 // part != nullptr: per-(ray, owner brick) fragments for the sort-last compositor instead of pixels
 static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, const TfK &tf,
                               const PartK *part, float *img, long long pitch_f, cudaStream_t st)
@@ -565,17 +572,17 @@ static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam,
     int rows;
     if (!have_z || n_x == 0) {
         make_lane_map(c, n, 0, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else if (n_x == 9) {
         make_lane_map(c, n, 2, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else {
         make_lane_map(c, n, 0, 1, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, rows, img, pitch_f, st);
         make_lane_map(c, n, 2, 2, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, rows, img, pitch_f, st);
         v->stats.kernel_launches += 2;
     }
     v->stats.path = 7;
@@ -796,7 +803,7 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     TfK tf; tf.table = v->d_tf; tf.scale = v->tf_scale; tf.bias = v->tf_bias;
     if (sort_last) rc = render_sort_last(v, c, cam, mode, tf, img, pitch_f, st);
     else if (v->out_of_core || v->desc.layout == VR_BRICKED_HALO1) rc = render_chain(v, c, cam, mode, ert, tf, img, pitch_f, st);
-    else if (v->opt_path == 1) rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
+    else if (v->opt_path == 1 || !lanes_addressable(v)) rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
     else rc = render_lanes(v, c, cam, mode, ert, tf, nullptr, img, pitch_f, st);
     if (rc != VR_OK) return rc;
     VR_CUDA(cudaGetLastError());
@@ -916,6 +923,9 @@ VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
     case VR_OPT_LANE_LAG:
         VR_REQUIRE(value >= 0 && value <= 1024, "VR_OPT_LANE_LAG: 0..1024 base planes (got %lld)", (long long)value);
         v->opt_lag = (int)value; return VR_OK;
+    case VR_OPT_FORCE_WIDE:
+        VR_REQUIRE(value == 0 || value == 1, "VR_OPT_FORCE_WIDE: 0 or 1 (got %lld)", (long long)value);
+        v->opt_wide = (int)value; return VR_OK;
     case VR_OPT_EMPTY_SKIP:
         VR_REQUIRE(value == 0 || value == 1, "VR_OPT_EMPTY_SKIP: 0 never, 1 when the transfer function has empty intervals (got %lld)", (long long)value);
         v->opt_skip = (int)value; return VR_OK;

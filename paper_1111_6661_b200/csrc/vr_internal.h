@@ -46,6 +46,13 @@ inline void vr_launch(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, 
 #else
 #define VR_TEST_COUNT(i) ((void)0)
 #endif
+// memory-traffic model of the emulation (tests/simt/traffic_model.py): addresses of the four row pointers of a sample
+#ifdef VR_SIMT_HOST
+#define VR_TRACE_CORNER_LOADS(active, base, p0, p1, p2, p3) \
+    do { if (::simt::g_trace) ::simt::trace_corner_loads(active, base, p0, p1, p2, p3); } while (0)
+#else
+#define VR_TRACE_CORNER_LOADS(active, base, p0, p1, p2, p3) ((void)0)
+#endif
 enum { VR_CNT_LEAP_CELL = 0, VR_CNT_LEAP_BLOCK = 1, VR_CNT_LEAP_REJECTED = 2, VR_CNT_LAG_WAIT = 3 };
 
 // dynamic shared memory of the CTA as an array of T
@@ -120,15 +127,16 @@ struct WorkK { int brick, tx, ty, pad; };   // one CTA of the brick kernel: 16x8
 
 struct BinsK { const unsigned int *offs; const unsigned int *list; int tiles_x, tile; };
 
-void launch_march_full(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, float *image,
+// force_wide: 64-bit element offsets even where 32 bits would do (VR_OPT_FORCE_WIDE, for the tests)
+void launch_march_full(int mode, bool ert, bool force_wide, const CamK &cam, const VolK &vol, const TfK &tf, float *image,
                        long long pitch_f, cudaStream_t st);
 void launch_march_bricks(int mode, bool wide, const CamK &cam, const VolK &vol, const TfK &tf, const BrickK *bricks,
                          const WorkK *work, int n_work, float *arena, cudaStream_t st);
 void launch_composite(int mode, const CamK &cam, const BrickK *bricks, BinsK bins, const float *arena, float *image,
                       long long pitch_f, cudaStream_t st);
 void launch_chain_init(int mode, int W, int H, float *image, long long pitch_f, cudaStream_t st);
-void launch_chain_brick(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, const BrickK &brick,
-                        float *image, long long pitch_f, cudaStream_t st);
+void launch_chain_brick(int mode, bool ert, bool force_wide, const CamK &cam, const VolK &vol, const TfK &tf,
+                        const BrickK &brick, float *image, long long pitch_f, cudaStream_t st);
 void launch_chain_finish(int W, int H, float *image, long long pitch_f, cudaStream_t st);
 
 // ---------------------------------------------------------------- lane-mapped ray casting (vr_lanes.cu)
@@ -168,7 +176,8 @@ struct PartK {
 
 // part != nullptr: write per-(ray, owner brick) fragments instead of pixels (no ERT, C.7)
 void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
-                 const MacroK &macro, const PartK *part, int rows, float *image, long long pitch_f, cudaStream_t st);
+                 const MacroK &macro, const PartK *part, bool force_wide, int rows, float *image, long long pitch_f,
+                 cudaStream_t st);
 void launch_fragment_init(int mode, float *arena, unsigned long long n_frag, int grid, cudaStream_t st);
 void launch_transpose_xz(const float *in, float *out, int nx, int ny, int nz, cudaStream_t st);
 

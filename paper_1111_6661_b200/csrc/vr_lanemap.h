@@ -20,6 +20,7 @@ struct LaneMapK {
     int cls;            // pixels this launch renders: 0 all, 1 those with |d_x| <= |d_z|, 2 those with |d_x| > |d_z|
     int lag;            // 0 off; else a lane more than `lag` base planes ahead of the slowest active lane waits
     int paxis, psign;   // principal axis of the view and the sign of travel along it (progress measure of `lag`)
+    int w[3];           // psign on paxis, 0 elsewhere: progress of a sample = w . (ix, iy, iz)
 };
 
 inline int lane_row_offset(float sigma, int p) { return (int)floorf(fmaf(sigma, (float)p, 0.5f)); }
@@ -56,6 +57,7 @@ inline void make_lane_map(const vr_camera *cam, const int n[3], int fast, int cl
     if (pa == fast) pa = fast == 0 ? 2 : 0;                           // cls 0 on a copy whose fast axis is principal
     M.paxis = pa;
     M.psign = g[pa] >= 0.0 ? 1 : -1;
+    for (int a = 0; a < 3; ++a) M.w[a] = a == pa ? M.psign : 0;
     M.cls = cls;
     M.lag = lag;
     const int other = 3 - pa - fast;                                  // the in-plane axis that is not the fast one

@@ -67,12 +67,25 @@ __device__ __forceinline__ void composite_p(float4 rgba, float &Cr, float &Cg, f
 // the 8 corners of base index (ix,iy,iz): FAST = the axis with element stride 1 (0: x-fastest array,
 // 2: z-fastest copy); sa, sb = element strides of the other two axes in ascending axis order
 template <bool WIDE, int FAST>
+__device__ __forceinline__ const float *cell_pointer(const LaneVolK &V, int ix, int iy, int iz)
+{
+    // offset = slow index * slow stride + (middle index * middle stride + fast index): the bracket is an offset
+    // inside one plane and the slow stride is a plane size, both < 2^32 (checked by launch_rows), so the only
+    // 64-bit operation of the WIDE case is one 32 x 32 -> 64-bit multiply-add (indices are >= 0 by C.3)
+    const unsigned int in_plane = FAST == 0 ? (unsigned int)iy * (unsigned int)V.sa + (unsigned int)ix
+                                            : (unsigned int)iy * (unsigned int)V.sb + (unsigned int)iz;
+    const unsigned int slow = FAST == 0 ? (unsigned int)iz : (unsigned int)ix;
+    const unsigned int s_slow = FAST == 0 ? (unsigned int)V.sb : (unsigned int)V.sa;
+    const float *p;
+    if (WIDE) p = V.base + ((unsigned long long)slow * s_slow + in_plane);
+    else p = V.base + (slow * s_slow + in_plane);
+    return p;
+}
+
+template <bool WIDE, int FAST>
 __device__ __forceinline__ float sample_cell(const LaneVolK &V, int ix, int iy, int iz, float fx, float fy, float fz)
 {
-    const int ia = FAST == 0 ? iy : ix, ib = FAST == 0 ? iz : iy, iu = FAST == 0 ? ix : iz;
-    const float *p;
-    if (WIDE) p = V.base + ((long long)ib * V.sb + (long long)ia * V.sa + iu);
-    else p = V.base + ((unsigned int)ib * (unsigned int)V.sb + (unsigned int)ia * (unsigned int)V.sa + (unsigned int)iu);
+    const float *p = cell_pointer<WIDE, FAST>(V, ix, iy, iz);
     const float *pa = p + V.sa, *pb = p + V.sb, *pab = pb + V.sa;
     const float q00 = __ldg(p), q01 = __ldg(p + 1);          // (a, b) = (0, 0): unit-stride neighbours
     const float q10 = __ldg(pa), q11 = __ldg(pa + 1);        // a + 1
@@ -159,7 +172,7 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__re
         alive = mine && hit && r.t_exit < CUDART_INF_F;
     }
     if (!__any_sync(0xffffffffu, mine)) return;
-    if (!alive) { r.t_first = 0.0f; r.t_exit = 0.0f; r.d[0] = r.d[1] = r.d[2] = 0.0f; r.oc[0] = r.oc[1] = r.oc[2] = 0.0f; }
+    if (!alive) { r.t_first = 0.0f; r.t_exit = -CUDART_INF_F; r.d[0] = r.d[1] = r.d[2] = 0.0f; r.oc[0] = r.oc[1] = r.oc[2] = 0.0f; }
     float cr = 0.0f, cg = 0.0f, cb = 0.0f, T = 1.0f, m = -CUDART_INF_F;
     float kf = 0.0f;
     const int lag = M.lag;
@@ -170,9 +183,10 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__re
 #pragma unroll
         for (int a = 0; a < 3; ++a) inv[a] = 1.0f / r.d[a];          // only used by the leap estimate (d_a != 0 checked there)
     }
+    // a ray that is not marched (miss, other class, outside the image) or has terminated has t_exit below every t_k
     for (;;) {
         const float t = __fmaf_rn(kf, cam.step, r.t_first);
-        alive = alive && t < r.t_exit;                               // C.2: sample k exists iff t_k < t_exit
+        alive = t < r.t_exit;                                        // C.2: sample k exists iff t_k < t_exit
         if (!__any_sync(0xffffffffu, alive)) break;
         int ix, iy, iz;
         float fx, fy, fz;
@@ -181,12 +195,17 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__re
         axis_cell(t, r.d[2], r.oc[2], V.nz, iz, fz);
         bool go = alive;
         if (lag > 0) {
-            const int ip = M.paxis == 0 ? ix : M.paxis == 1 ? iy : iz;
-            const int prog = M.psign >= 0 ? ip : -ip;
+            const int prog = ix * M.w[0] + iy * M.w[1] + iz * M.w[2];        // +- the base index along the principal axis
             const int slowest = __reduce_min_sync(0xffffffffu, alive ? prog : INT_MAX);
             go = alive && prog - slowest <= lag;
             if (alive && !go) VR_TEST_COUNT(VR_CNT_LAG_WAIT);
         }
+#ifdef VR_SIMT_HOST
+        if (!SKIP) {
+            const float *p = cell_pointer<WIDE, FAST>(V, ix, iy, iz);
+            VR_TRACE_CORNER_LOADS(go, V.base, p, p + V.sa, p + V.sb, p + V.sb + V.sa);
+        }
+#endif
         if (PART && go && (ix < blo[0] || ix > bhi[0] || iy < blo[1] || iy > bhi[1] || iz < blo[2] || iz > bhi[2])) {
             if (cur >= 0) flush_fragment<MODE>(P, cur, i, j, cr, cg, cb, T, m);
             const int bx = ix / P.B, by = iy / P.B, bz = iz / P.B;
@@ -204,7 +223,7 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__re
                 if (MODE == VR_MIP) m = fmaxf(m, s);
                 else {
                     composite_p(classify_s(tf_s, tf.scale, tf.bias, s), cr, cg, cb, T);
-                    if (ERT && T <= cam.t_min) alive = false;       // stop AFTER compositing this sample (C.5)
+                    if (ERT && T <= cam.t_min) r.t_exit = -CUDART_INF_F;      // stop AFTER compositing this sample (C.5)
                 }
                 kf = __fadd_rn(kf, 1.0f);                            // exact: k < 2^24
             } else                                                   // leap to the end of the empty cell (or block of cells)
@@ -254,7 +273,8 @@ k_transpose_xz(const float *__restrict__ in, float *__restrict__ out, int nx, in
 }  // namespace
 
 void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
-                 const MacroK &macro, const PartK *part, int rows, float *image, long long pitch_f, cudaStream_t st)
+                 const MacroK &macro, const PartK *part, bool force_wide, int rows, float *image, long long pitch_f,
+                 cudaStream_t st)
 {
     const int n_lane = map.lane_axis == 0 ? cam.width : cam.height;
     const dim3 g((unsigned)((n_lane + 31) / 32), (unsigned)((rows + kRowsPerCta - 1) / kRowsPerCta));
@@ -262,7 +282,7 @@ void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int f
     const unsigned long long span = (unsigned long long)((fast == 0 ? vol.nz : vol.ny) - 1) * (unsigned long long)vol.sb +
                                     (unsigned long long)((fast == 0 ? vol.ny : vol.nx) - 1) * (unsigned long long)vol.sa +
                                     (unsigned long long)(fast == 0 ? vol.nx : vol.nz);
-    const bool wide = span > 0xffffffffull;
+    const bool wide = force_wide || span > 0xffffffffull;
     const bool skip = mode == VR_EA && macro.flag != nullptr && !part;
     PartK P;
     if (part) P = *part;

@@ -46,6 +46,7 @@ __device__ __forceinline__ float sample_at(const VolK &V, const Ray &r, float t)
     if (WIDE) p = V.base + ((long long)iz * V.sz + (long long)iy * V.sy + ix);
     else p = V.base + ((unsigned int)iz * (unsigned int)V.sz + (unsigned int)iy * (unsigned int)V.sy + (unsigned int)ix);
     const float *pz = p + V.sz;
+    VR_TRACE_CORNER_LOADS(true, V.base, p, p + V.sy, pz, pz + V.sy);
     const float v000 = __ldg(p), v100 = __ldg(p + 1);
     const float v010 = __ldg(p + V.sy), v110 = __ldg(p + V.sy + 1);
     const float v001 = __ldg(pz), v101 = __ldg(pz + 1);
@@ -221,11 +222,11 @@ inline bool needs_wide(const VolK &V)
 
 }  // namespace
 
-void launch_march_full(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, float *image,
+void launch_march_full(int mode, bool ert, bool force_wide, const CamK &cam, const VolK &vol, const TfK &tf, float *image,
                        long long pitch_f, cudaStream_t st)
 {
     const dim3 g = tiles(cam.width, cam.height);
-    const bool wide = needs_wide(vol);
+    const bool wide = force_wide || needs_wide(vol);
 #define VR_LAUNCH(M, E, Wd) vr_launch(k_march_full<M, E, Wd>, g, kThreads, 0, st, cam, vol, tf, image, pitch_f)
     if (mode == VR_MIP) { if (wide) VR_LAUNCH(VR_MIP, false, true); else VR_LAUNCH(VR_MIP, false, false); }
     else if (ert) { if (wide) VR_LAUNCH(VR_EA, true, true); else VR_LAUNCH(VR_EA, true, false); }
@@ -258,14 +259,14 @@ void launch_chain_init(int mode, int W, int H, float *image, long long pitch_f, 
     else vr_launch(k_chain_init<VR_EA>, g, 256, 0, st, W, H, image, pitch_f);
 }
 
-void launch_chain_brick(int mode, bool ert, const CamK &cam, const VolK &vol, const TfK &tf, const BrickK &brick,
-                        float *image, long long pitch_f, cudaStream_t st)
+void launch_chain_brick(int mode, bool ert, bool force_wide, const CamK &cam, const VolK &vol, const TfK &tf,
+                        const BrickK &brick, float *image, long long pitch_f, cudaStream_t st)
 {
     const dim3 g = tiles(brick.x1 - brick.x0, brick.y1 - brick.y0);
     if (g.x == 0 || g.y == 0) return;
     VolK V = vol;
     V.base = brick.base; V.sy = brick.sy; V.sz = brick.sz; V.ox = brick.ox; V.oy = brick.oy; V.oz = brick.oz;
-    const bool wide = (unsigned long long)V.sz * (unsigned long long)(V.sz / (V.sy ? V.sy : 1) + 2) > 0xffffffffull;   // slot of E^3 elements
+    const bool wide = force_wide || (unsigned long long)V.sz * (unsigned long long)(V.sz / (V.sy ? V.sy : 1) + 2) > 0xffffffffull;   // slot of E^3 elements
 #define VR_LAUNCH(M, E, Wd) vr_launch(k_chain_brick<M, E, Wd>, g, kThreads, 0, st, cam, V, tf, brick, image, pitch_f)
     if (mode == VR_MIP) { if (wide) VR_LAUNCH(VR_MIP, false, true); else VR_LAUNCH(VR_MIP, false, false); }
     else if (ert) { if (wide) VR_LAUNCH(VR_EA, true, true); else VR_LAUNCH(VR_EA, true, false); }

@@ -29,6 +29,9 @@ def lib():
         l.simt_free.argtypes = [C.c_void_p]
         l.simt_device_bytes_in_use.restype = C.c_size_t
         l.simt_set_device_capacity.argtypes = [C.c_size_t]
+        l.simt_trace.argtypes = [C.c_int]
+        l.simt_trace_stat.restype = C.c_ulonglong
+        l.simt_trace_stat.argtypes = [C.c_int]
         l.simt_counter.restype = C.c_ulonglong
         l.simt_counter.argtypes = [C.c_int]
         _lib = l

@@ -34,6 +34,8 @@ namespace simt {
 Builtins g_cur;
 unsigned char *g_dyn_smem = nullptr;
 unsigned long long g_counters[16] = {};
+int g_trace = 0;
+unsigned long long g_trace_stats[8] = {};
 
 namespace {
 
@@ -226,6 +228,35 @@ const WarpTable &warp_exchange(uint32_t mask, uint64_t value)
     return w.table[(my_gen + 1) & 1u];
 }
 
+void trace_corner_loads(bool active, const void *base, const void *p0, const void *p1, const void *p2, const void *p3)
+{
+    const void *ptr[4] = { p0, p1, p2, p3 };
+    const int lane = g_running & 31;
+    for (int r = 0; r < 4; ++r) {
+        const uint64_t off = active ? (uint64_t)((const char *)ptr[r] - (const char *)base) : ~0ull;
+        const WarpTable &t = warp_exchange(0u, off);                 // every live lane of the warp arrives here
+        int first = -1, n_act = 0;
+        for (int l = 0; l < 32; ++l) if ((t.present >> l & 1u) && t.v[l] != ~0ull) { if (first < 0) first = l; ++n_act; }
+        if (lane != first) continue;                                 // one lane does the counting
+        if (r == 0) { g_trace_stats[0] += 1; g_trace_stats[1] += (unsigned long long)n_act; }
+        for (int e = 0; e < 2; ++e) {                                // the loads of p and p + 1 element
+            uint64_t lines[32], sectors[32];
+            int nl = 0, ns = 0;
+            for (int l = 0; l < 32; ++l) {
+                if (!(t.present >> l & 1u) || t.v[l] == ~0ull) continue;
+                const uint64_t a = t.v[l] + 4u * (unsigned)e, ln = a >> 7, sc = a >> 5;
+                bool seen = false;
+                for (int k = 0; k < nl; ++k) seen = seen || lines[k] == ln;
+                if (!seen) lines[nl++] = ln;
+                seen = false;
+                for (int k = 0; k < ns; ++k) seen = seen || sectors[k] == sc;
+                if (!seen) sectors[ns++] = sc;
+            }
+            g_trace_stats[2] += 1; g_trace_stats[3] += (unsigned long long)nl; g_trace_stats[4] += (unsigned long long)ns;
+        }
+    }
+}
+
 int cta_barrier(int pred, int mode)
 {
     const int me = g_running;
@@ -308,6 +339,8 @@ __attribute__((visibility("default"))) size_t simt_device_bytes_in_use(void) { r
 // event counters the kernels bump through VR_TEST_COUNT (vr_internal.h): tests assert that a code path really ran
 __attribute__((visibility("default"))) unsigned long long simt_counter(int i) { return i >= 0 && i < 16 ? simt::g_counters[i] : 0; }
 __attribute__((visibility("default"))) void simt_reset_counters(void) { for (auto &c : simt::g_counters) c = 0; }
+__attribute__((visibility("default"))) void simt_trace(int on) { simt::g_trace = on; for (auto &c : simt::g_trace_stats) c = 0; }
+__attribute__((visibility("default"))) unsigned long long simt_trace_stat(int i) { return i >= 0 && i < 8 ? simt::g_trace_stats[i] : 0; }
 __attribute__((visibility("default"))) void simt_set_device_capacity(size_t n) { g_device_capacity = n; }
 
 cudaError_t cudaMalloc(void **p, size_t n)

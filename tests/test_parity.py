@@ -362,6 +362,31 @@ def test_zfast_copy_skipped_when_memory_is_short(be):
     assert np.array_equal(g, O.render(v, cam, O.MIP).image)
 
 
+@pytest.mark.parametrize("how", ["lanes", "tiles", "sort_last", "chain"])
+def test_64_bit_offsets_at_small_size(be, how):
+    """VR_OPT_FORCE_WIDE: the 64-bit voxel-offset arithmetic that volumes of more than 2^32 voxels (cfg4) run, at a
+    size the oracle and the host emulation finish in seconds; z- and x-travelling views (both volume copies)."""
+    n, B = (52, 40, 61), 16
+    v = W.make_cube(W.Recipe(*n, seed=77, n_sources=4))
+    s = O.minmax_hist(v)
+    R = float(max(abs(s.vmin), abs(s.vmax)))
+    tf = W.tf_opaque(n, 0.5)
+    views = [c for k, c in _axis_views(n, False) if k in ("persp0", "persp4", "persp6", "ortho_x")]
+    data = be.dev(W.retile_halo(v, B)) if how == "chain" else be.dev(v)
+    with vr.Volume(data, n, brick=B, layout=vr.VR_BRICKED_HALO1 if how == "chain" else vr.VR_LINEAR) as vol:
+        vol.set_option(vr.VR_OPT_FORCE_WIDE, 1)
+        if how == "tiles":
+            vol.set_option(vr.VR_OPT_RENDER_PATH, vr.VR_PATH_RAY_MAJOR)
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for cam in views:
+            sl = how == "sort_last"
+            cam2 = cam.with_(ert_alpha=0.0 if sl else 0.99, flags=W.cameras.VR_SORT_LAST if sl else 0)
+            oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax, brick=B if sl else 0)
+            assert np.array_equal(render(be, vol, cam2, vr.VR_EA), oe.image)
+            om = O.render(v, cam2, O.MIP, brick=B if sl else 0)
+            assert np.array_equal(render(be, vol, cam2, vr.VR_MIP), om.image)
+
+
 def test_mixed_camera_renders(be):
     """A camera whose origins AND directions vary per pixel (neither perspective nor orthographic)."""
     n = (32, 32, 32)
@@ -377,7 +402,8 @@ def test_mixed_camera_renders(be):
 def test_set_option_rejects_bad_values(be):
     v = W.make_cube(W.Recipe(16, 16, 16, seed=1))
     with vr.Volume(be.dev(v), (16, 16, 16)) as vol:
-        for opt, val in ((vr.VR_OPT_RENDER_PATH, 5), (vr.VR_OPT_ZFAST_COPY, 2), (vr.VR_OPT_LANE_LAG, -1), (77, 0)):
+        for opt, val in ((vr.VR_OPT_RENDER_PATH, 5), (vr.VR_OPT_ZFAST_COPY, 2), (vr.VR_OPT_LANE_LAG, -1),
+                         (vr.VR_OPT_EMPTY_SKIP, 2), (vr.VR_OPT_FORCE_WIDE, -1), (77, 0)):
             with pytest.raises(vr.VrError) as e:
                 vol.set_option(opt, val)
             assert e.value.status == vr.VR_ERR_INVALID_ARG
