@@ -674,15 +674,21 @@ VR_API vr_status vr_create_volume(const vr_volume_desc *d, vr_volume **out)
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { vr_status r__ = cuda_fail(e__, #call); free_volume(v); return r__; } } while (0)
 
     VR_FAIL_CUDA(cudaGetDevice(&v->device));
-    VR_FAIL_CUDA(cudaDeviceGetAttribute(&v->sm_count, cudaDevAttrMultiProcessorCount, v->device));
     cudaPointerAttributes attr;
     VR_FAIL_CUDA(cudaPointerGetAttributes(&attr, d->data));
     if (d->location == VR_DEVICE) {
         if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged) {
             free_volume(v); set_error("location VR_DEVICE but data is not a device pointer"); return VR_ERR_INVALID_ARG;
         }
+        // the handle lives on the device that owns the data, whatever device is current in the calling thread
+        if (attr.type == cudaMemoryTypeDevice && attr.device != v->device) {
+            v->device = attr.device;
+            VR_FAIL_CUDA(cudaSetDevice(v->device));
+        }
         v->dev_data = d->data;
-    } else {
+    }
+    VR_FAIL_CUDA(cudaDeviceGetAttribute(&v->sm_count, cudaDevAttrMultiProcessorCount, v->device));
+    if (d->location != VR_DEVICE) {
         if (attr.type != cudaMemoryTypeHost) {
             free_volume(v); set_error("location VR_HOST_PINNED but data is not page-locked host memory"); return VR_ERR_INVALID_ARG;
         }
