@@ -387,6 +387,68 @@ def test_64_bit_offsets_at_small_size(be, how):
             assert np.array_equal(render(be, vol, cam2, vr.VR_MIP), om.image)
 
 
+@pytest.mark.parametrize("n", [(2, 5, 9), (64, 2, 33), (7, 40, 2), (2, 2, 2)])
+def test_degenerate_dimensions(be, n):
+    """An axis of length 2 (one cell: i0 is always 0 and the whole axis is 'outer half voxel'), every render path;
+    bricks larger than the cube and bricks of edge 2."""
+    v = W.make_cube(W.Recipe(*n, seed=101, n_sources=0))
+    s = O.minmax_hist(v)
+    tf = W.bake_tf(W.TF_HAZE_POINTS, 0.5, alpha_scale=20.0)
+    c = np.array(n, dtype=np.float64) / 2
+    m = float(max(n))
+    cams = [W.perspective_camera(c + np.array(e) * m * 1.5, c, (0, 1, 0), 50.0, 45, 37, step=0.3)
+            for e in ((1.2, 0.5, 0.8), (-0.3, 0.2, 1.5), (0.2, 1.6, 0.1))]
+    cams.append(W.ortho_axis_camera(n, 1, +1, step=0.5))
+    for path in (0, 1):
+        with vr.Volume(be.dev(v), n, brick=2) as vol:
+            vol.set_option(vr.VR_OPT_RENDER_PATH, path)
+            vol.set_transfer_function(tf, s.vmin, s.vmax)
+            for k, up in enumerate(cams):
+                for ert in (0.0, 0.9):
+                    oe = O.render(v, up.with_(ert_alpha=ert), O.EA, tf, s.vmin, s.vmax)
+                    assert np.array_equal(render(be, vol, up.with_(ert_alpha=ert), vr.VR_EA), oe.image), (n, path, k, ert)
+                om = O.render(v, up, O.MIP)
+                assert np.array_equal(render(be, vol, up, vr.VR_MIP), om.image), (n, path, k)
+                if up.is_perspective or up.is_orthographic:
+                    sl = up.with_(flags=W.cameras.VR_SORT_LAST)
+                    ob = O.render(v, sl, O.EA, tf, s.vmin, s.vmax, brick=2)
+                    assert np.array_equal(render(be, vol, sl, vr.VR_EA), ob.image), (n, path, k, "sort-last")
+    with vr.Volume(be.dev(v), n, brick=1000) as vol:               # one brick larger than the cube
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        sl = cams[0].with_(flags=W.cameras.VR_SORT_LAST)
+        assert np.array_equal(render(be, vol, sl, vr.VR_EA), O.render(v, sl, O.EA, tf, s.vmin, s.vmax, brick=1000).image)
+
+
+def test_rays_along_brick_planes_and_opaque_first_sample(be):
+    """Orthographic rays with d_a = 0 whose origin lies exactly on an ownership plane o_a = B b + 1/2 (every sample
+    sits on the boundary between two bricks: C.7 gives it to exactly one); alpha = 1 everywhere with ERT (K = 1:
+    the ray stops after its first sample, P7)."""
+    n, B = (32, 24, 40), 8
+    v = W.make_cube(W.Recipe(*n, seed=55, n_sources=2))
+    s = O.minmax_hist(v)
+    cam = W.ortho_axis_camera(n, 2, +1, step=0.5, width=8, height=6)   # pixel centres at x = 2, 6, .. ; y = 2, 6, ..
+    vec = cam.vectors()
+    o0 = vec[0].copy(); o0[0] += 8.5 - 2.0; o0[1] += 8.5 - 2.0            # first pixel centre on the planes x = y = 8.5
+    cam = cam.with_(o0=o0, ou=np.array([8.0, 0, 0], np.float32), ov=np.array([0, 8.0, 0], np.float32), width=3, height=2)
+    tf = W.tf_haze(n, 0.5)
+    one = np.ones((256, 4), dtype=np.float32)
+    with vr.Volume(be.dev(v), n, brick=B) as vol:
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for flags in (0, W.cameras.VR_SORT_LAST):
+            c2 = cam.with_(flags=flags)
+            o = O.render(v, c2, O.EA, tf, s.vmin, s.vmax, brick=B if flags else 0)
+            assert o.n_order_mismatch == 0 and o.n_noncontig == 0
+            assert np.array_equal(render(be, vol, c2, vr.VR_EA), o.image), flags
+            om = O.render(v, c2, O.MIP, brick=B if flags else 0)
+            assert np.array_equal(render(be, vol, c2, vr.VR_MIP), om.image), flags
+        vol.set_transfer_function(one, s.vmin, s.vmax)
+        view = W.orbit_camera(n, 1, 8, 40, 30, step=0.5, ert_alpha=0.5)
+        o = O.render(v, view, O.EA, one, s.vmin, s.vmax)
+        assert (o.K_ert[o.K > 0] == 1).all()
+        g = render(be, vol, view, vr.VR_EA)
+        assert np.array_equal(g, o.image) and (g[o.K > 0] == 1.0).all()
+
+
 def test_mixed_camera_renders(be):
     """A camera whose origins AND directions vary per pixel (neither perspective nor orthographic)."""
     n = (32, 32, 32)
