@@ -143,13 +143,86 @@ def aggregate_value(units_per_rank: float, world: int, ms_step: float) -> float:
     return world * units_per_rank / (ms_step * 1e-3)
 
 
+# ---------------------------------------------------------------------------------- device rig
+_NP2TORCH = {"float32": "float32", "uint8": "uint8"}
+
+
+class TorchCudaRig:
+    """Everything bench.py needs from the device side — buffers, events on the launching stream, synchronisation —
+    behind one small object, so that tests/test_bench_host.py can execute the whole measurement flow (and the JSON
+    line it assembles) against the host emulation of the library with a rig of the same interface."""
+    name = "cuda"
+
+    def __init__(self, local: int):
+        import torch
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+        torch.cuda.set_device(local)
+        self.torch, self.local = torch, local
+        self.stream = torch.cuda.current_stream()
+        self.stream_arg = self.stream                       # what the binding's `stream=` takes
+
+    def _dt(self, dtype):
+        return getattr(self.torch, _NP2TORCH[np.dtype(dtype).name])
+
+    def host_empty(self, shape, dtype=np.float32, pinned=True):
+        return self.torch.empty(tuple(shape), dtype=self._dt(dtype), pin_memory=pinned)
+
+    def dev_empty(self, shape, dtype=np.float32):
+        return self.torch.empty(tuple(shape), dtype=self._dt(dtype), device="cuda")
+
+    def to_device(self, host):
+        return host.cuda()
+
+    def as_numpy(self, host):
+        return host.numpy()
+
+    def read(self, t):
+        """Synchronise and return the bytes of a device or pinned-host buffer as a numpy array."""
+        self.torch.cuda.synchronize()
+        return (t.cpu() if t.is_cuda else t).numpy()
+
+    def event(self):
+        return self.torch.cuda.Event(enable_timing=True)
+
+    def record(self, e):
+        e.record(self.stream)
+
+    def elapsed_ms(self, a, b) -> float:
+        return float(a.elapsed_time(b))
+
+    def synchronize(self):
+        self.torch.cuda.synchronize()
+
+    def stream_synchronize(self):
+        self.stream.synchronize()
+
+    def empty_cache(self):
+        self.torch.cuda.empty_cache()
+
+    def copy_h2d(self, d, h):
+        d.copy_(h, non_blocking=True)
+
+    def clock_sampler(self):
+        return ClockSampler(physical_gpu_index(self.local))
+
+
+def read_summary(rig, buf, nbins: int = 256):
+    import paper_1111_6661_b200 as vr
+    raw = np.ascontiguousarray(rig.read(buf)).tobytes()[: 32 + 8 * nbins]
+    return np.frombuffer(raw, dtype=vr.summary_dtype(nbins))[0]
+
+
 # ---------------------------------------------------------------------------------- workload
-def make_host_cube(cfg, pinned=True):
+def make_host_cube(cfg, rig=None, pinned=True):
     """The config's seeded cube in (pinned) host memory, filled in z-slabs by the shared generator."""
-    import torch
     import workload as W
     nx, ny, nz = cfg.dims
-    t = torch.empty((nz, ny, nx), dtype=torch.float32, pin_memory=pinned)
+    if rig is None:
+        import torch
+        t = torch.empty((nz, ny, nx), dtype=torch.float32, pin_memory=pinned)
+    else:
+        t = rig.host_empty((nz, ny, nx), np.float32, pinned)
     gen = W.CubeGenerator(cfg.recipe)
     slab = max(1, (1 << 28) // (nx * ny))
     for z0 in range(0, nz, slab):
@@ -193,14 +266,17 @@ def cpu_oracle_rate(cfg, host_np, tf, vmin, vmax, budget_s=15.0, view=0):
             "seconds": dt, "n_samples": int(n_nom)}
 
 
-def run_reference(args):
+def run_reference(args, cfg=None):
     """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
-        return
+        return None
     import workload as W
     import oracle as O
-    cfg = W.get_config(args.config)
-    host = make_host_cube(cfg, pinned=False).numpy()
+    if cfg is None:
+        cfg = W.get_config(args.config)
+        if cfg.out_of_core:                      # the linear cube of cfg5 does not fit the host: same cut as our arm
+            cfg, _ = ooc_config(cfg, args.ooc_nz)
+    host = make_host_cube(cfg, None, pinned=False).numpy()
     s = O.minmax_hist(host[: max(2, min(host.shape[0], (1 << 27) // (host.shape[1] * host.shape[2])))])
     tf = W.tf_haze(cfg.dims, cfg.step)
     budget = 45.0 / max(args.steps + args.warmup, 1)
@@ -221,6 +297,7 @@ def run_reference(args):
             "e2e": {"value": value, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+    return line
 
 
 def config_block(cfg, note=""):
@@ -234,32 +311,32 @@ def config_block(cfg, note=""):
 
 
 # ---------------------------------------------------------------------------------- our arm
-def run_ours(args):
-    import torch
+def run_ours(args, rig=None, cfg=None):
+    """`rig` / `cfg`: the emulated rig and a scaled config of tests/test_bench_host.py; None = B200 and --config."""
     import paper_1111_6661_b200 as vr
     import workload as W
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
-    torch.cuda.set_device(local)
+    if rig is None:
+        rig = TorchCudaRig(local)
     dist = None
     if world > 1:
+        import torch
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    cfg = W.get_config(args.config)
+    if cfg is None:
+        cfg = W.get_config(args.config)
     if cfg.out_of_core:
         if dist is not None:
             dist.destroy_process_group()
-        return run_ours_ooc(args, cfg)
+        return run_ours_ooc(args, cfg, rig)
     nx, ny, nz = cfg.dims
     n_vox = nx * ny * nz
-    host = make_host_cube(cfg, pinned=True)
-    dev = host.cuda()
-    stream = torch.cuda.current_stream()
+    host = make_host_cube(cfg, rig, pinned=True)
+    dev = rig.to_device(host)
     modes = modes_of(cfg)
     view_ids = list(range(cfg.n_views))
     if args.views > 0:
@@ -277,52 +354,52 @@ def run_ours(args):
         vol.set_option(vr.VR_OPT_LANE_LAG, args.lag)
     if args.no_zcopy:
         vol.set_option(vr.VR_OPT_ZFAST_COPY, 0)
-    sbuf = torch.empty(32 + 8 * 256, dtype=torch.uint8, device="cuda")
-    s = vr.Volume.read_summary(vol.minmax_histogram(256, out=sbuf))
+    sbuf = rig.dev_empty((32 + 8 * 256,), np.uint8)
+    vol.minmax_histogram(256, out=sbuf, stream=rig.stream_arg)
+    s = read_summary(rig, sbuf)
     vmin, vmax = float(s["vmin"]), float(s["vmax"])
     tf = W.tf_haze(cfg.dims, cfg.step)
-    images = {m: torch.empty((cfg.height, cfg.width, 4) if m == vr.VR_EA else (cfg.height, cfg.width),
-                             dtype=torch.float32, device="cuda") for m in modes}
+    images = {m: rig.dev_empty((cfg.height, cfg.width, 4) if m == vr.VR_EA else (cfg.height, cfg.width)) for m in modes}
 
     ev_pairs = []                                    # (start, end) around every vr_render of the timed region
 
     def step(record=False):
-        vol.minmax_histogram(256, out=sbuf)
+        vol.minmax_histogram(256, out=sbuf, stream=rig.stream_arg)
         vol.set_transfer_function(tf, vmin, vmax)
         n = 0
         for m in modes:
             for c in cam_structs:
                 if record:
-                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a.record(stream)
-                vol.render(c, m, out=images[m])
+                    a, b = rig.event(), rig.event()
+                    rig.record(a)
+                vol.render(c, m, out=images[m], stream=rig.stream_arg)
                 if record:
-                    b.record(stream); ev_pairs.append((a, b))
+                    rig.record(b); ev_pairs.append((a, b))
                 n += vol.stats()["kernel_launches"]
         return n
 
     def barrier():
-        torch.cuda.synchronize()
+        rig.synchronize()
         if dist is not None:
             dist.barrier()
-            torch.cuda.synchronize()
+            rig.synchronize()
 
     for _ in range(args.warmup):
         step()
     barrier()
-    clocks = ClockSampler(physical_gpu_index(local))
+    clocks = rig.clock_sampler()
     clocks.start()
     launches0 = vol.stats()["total_kernel_launches"]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
+    e0, e1 = rig.event(), rig.event()
+    rig.record(e0)
     for _ in range(args.steps):
         step(record=True)
-    e1.record(stream)
+    rig.record(e1)
     barrier()
     clk = clocks.finish()
-    ms_total = e0.elapsed_time(e1)
+    ms_total = rig.elapsed_ms(e0, e1)
     launches = vol.stats()["total_kernel_launches"] - launches0
-    render_ms = [a.elapsed_time(b) for a, b in ev_pairs]
+    render_ms = [rig.elapsed_ms(a, b) for a, b in ev_pairs]
     path = vol.stats()["path"]
     zfast = vol.stats()["zfast_copy"]
     # cold cameras: one orbit at azimuths none of the steps above has seen (an interactively moving camera);
@@ -332,50 +409,50 @@ def run_ours(args):
         for v_i in view_ids:
             c = vr.make_camera(W.orbit_camera(cfg.dims, v_i + 0.37, cfg.n_views, cfg.width, cfg.height, step=cfg.step,
                                               ert_alpha=cfg.ert_alpha))
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream); vol.render(c, modes[0], out=images[modes[0]]); b.record(stream)
+            a, b = rig.event(), rig.event()
+            rig.record(a); vol.render(c, modes[0], out=images[modes[0]], stream=rig.stream_arg); rig.record(b)
             cold_ms.append((a, b))
-        torch.cuda.synchronize()
-        cold_ms = [a.elapsed_time(b) for a, b in cold_ms]
+        rig.synchronize()
+        cold_ms = [rig.elapsed_ms(a, b) for a, b in cold_ms]
     ms_total = max_over_ranks([ms_total], dist, "cuda")[0]
     ms_step = ms_total / args.steps
     value = aggregate_value(samples_step, world, ms_step)
 
     # ---- end to end through the C ABI with host buffers (every step uploads the cube)
-    h_sum = torch.empty(32 + 8 * 256, dtype=torch.uint8).pin_memory()
-    h_img = {m: torch.empty(tuple(images[m].shape), dtype=torch.float32).pin_memory() for m in modes}
+    h_sum = rig.host_empty((32 + 8 * 256,), np.uint8)
+    h_img = {m: rig.host_empty(tuple(images[m].shape)) for m in modes}
 
     def e2e_step():
         with vr.Volume(host, cfg.dims, brick=cfg.brick, n_copy_streams=4) as hv:
-            hv.minmax_histogram(256, out=h_sum)
+            hv.minmax_histogram(256, out=h_sum, stream=rig.stream_arg)
             h2d = hv.stats()["h2d_bytes"]
-            torch.cuda.current_stream().synchronize()
-            hs = vr.Volume.read_summary(h_sum)
+            rig.stream_synchronize()
+            hs = read_summary(rig, h_sum)
             hv.set_transfer_function(tf, float(hs["vmin"]), float(hs["vmax"]))
             d2h = 32 + 8 * 256
             for m in modes:
                 for c in cam_structs:
-                    hv.render(c, m, out=h_img[m])
+                    hv.render(c, m, out=h_img[m], stream=rig.stream_arg)
                     d2h += hv.stats()["d2h_bytes"]
-            torch.cuda.current_stream().synchronize()
+            rig.stream_synchronize()
         return h2d, d2h
 
     vol.close()
     del dev
-    torch.cuda.empty_cache()
+    rig.empty_cache()
     e2e_steps = max(1, min(args.steps, 3))
     h2d = d2h = 0
     e2e_ms = float("nan")
     if not args.no_e2e:
         e2e_step()
         barrier()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
+        a, b = rig.event(), rig.event()
+        rig.record(a)
         for _ in range(e2e_steps):
             h2d, d2h = e2e_step()
-        b.record(stream)
+        rig.record(b)
         barrier()
-        e2e_ms = a.elapsed_time(b)
+        e2e_ms = rig.elapsed_ms(a, b)
     e2e_ms = max_over_ranks([e2e_ms], dist, "cuda")[0]
     e2e_value = aggregate_value(samples_step, world, e2e_ms / e2e_steps)
 
@@ -384,7 +461,7 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (the ray-march kernel: one launch per vr_render on path 1)
+    # ---- roofline of the dominant kernel (the ray-march kernel: one or two launches per vr_render)
     hbm_peak, sm_max_mhz, peak_src = measured_peaks()
     k_ms = float(np.mean(render_ms))
     ea_frac = sum(1 for m in modes if m == vr.VR_EA) / len(modes)
@@ -404,7 +481,8 @@ def run_ours(args):
                 "algorithmic_slots_per_sample": slots, "floor_ms": alu_floor_ms}
     alu_roof["frac"] = alu_roof["achieved"] / alu_roof["peak"]
     primary, other = (alu_roof, hbm_roof) if alu_floor_ms > hbm_floor_ms else (hbm_roof, alu_roof)
-    kname = {1: "k_march_full (ray-major tiles)", 2: "k_march_bricks + k_composite (sort-last)",
+    kname = {1: "k_march_full (ray-major tiles)",
+             2: "k_rows<PART> + k_composite (sort-last: one lane-mapped march per frame writes the per-brick fragments)",
              7: "k_rows (lane-mapped rows; one or two launches per vr_render)"}.get(path, f"vr_render path {path}")
     primary = dict(primary, kernel=kname, kernel_ms=k_ms, launches_timed=len(render_ms), zfast_copy=int(zfast))
 
@@ -427,12 +505,13 @@ def run_ours(args):
             "effective_hbm_gbs_per_frame": 4.0 * n_vox / (k_ms * 1e-3) / 1e9,
             "samples_per_step": int(samples_step)}
     if world == 1 and not args.no_cpu:
-        line["cpu_baseline"] = cpu_oracle_rate(cfg, host.numpy(), tf, vmin, vmax, budget_s=args.cpu_seconds)
+        line["cpu_baseline"] = cpu_oracle_rate(cfg, rig.as_numpy(host), tf, vmin, vmax, budget_s=args.cpu_seconds)
     else:
         line["cpu_baseline"] = None
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+    return line
 
 
 # ---------------------------------------------------------------------------------- out-of-core arm (cfg5)
@@ -466,111 +545,112 @@ def ooc_config(cfg, nz_arg: int):
     return replace(cfg, recipe=rec, name=f"{cfg.name}@nz{nz_arg}"), f"spectral axis cut from {nz} to {nz_arg} channels: the box cannot pin the full 209 GB"
 
 
-def measure_h2d_peak(stream) -> float:
+def measure_h2d_peak(rig, nbytes: int = 1 << 30) -> float:
     """Host-link peak as SURVEY 8(d) defines it: pinned 1 GiB cudaMemcpyAsync, best of 10, GB/s."""
-    import torch
-    h = torch.empty(1 << 30, dtype=torch.uint8).pin_memory()
-    d = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    h = rig.host_empty((nbytes,), np.uint8)
+    d = rig.dev_empty((nbytes,), np.uint8)
     best = 0.0
     for _ in range(10):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream); d.copy_(h, non_blocking=True); b.record(stream); torch.cuda.synchronize()
-        best = max(best, (1 << 30) / (a.elapsed_time(b) * 1e-3) / 1e9)
+        a, b = rig.event(), rig.event()
+        rig.record(a); rig.copy_h2d(d, h); rig.record(b); rig.synchronize()
+        best = max(best, nbytes / (max(rig.elapsed_ms(a, b), 1e-6) * 1e-3) / 1e9)
     del h, d
+    rig.empty_cache()
     return best
 
 
-def run_ours_ooc(args, cfg):
+def run_ours_ooc(args, cfg, rig):
     """cfg5: the cube lives in pinned host memory as brick-major 256^3(+1 halo) bricks; a fixed part of the brick
     pool stays resident, the rest is streamed per frame in view order on 4 copy streams (A5).  `value` times steps
     on one handle (resident part already loaded); `e2e` creates the handle inside every step."""
-    import torch
     import paper_1111_6661_b200 as vr
     import workload as W
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
     dist = None
     if world > 1:
+        import torch
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    cfg, size_note = ooc_config(cfg, args.ooc_nz)
+    if cfg.number == 5 and cfg.name == "cfg5":
+        cfg, size_note = ooc_config(cfg, args.ooc_nz)
+    else:
+        size_note = "scaled test config"
     nx, ny, nz = cfg.dims
     B = cfg.brick
     n_el = W.bricked_halo_elems(cfg.dims, B)
-    host = torch.empty(n_el, dtype=torch.float32, pin_memory=True)
+    host = rig.host_empty((n_el,), np.float32, pinned=True)
     W.fill_bricked_halo_ptr(cfg.recipe, B, host.data_ptr())
     cube_bytes = 4 * n_el
     resident = int(args.ooc_resident_frac * cube_bytes)
-    stream = torch.cuda.current_stream()
-    link_peak = measure_h2d_peak(stream)
+    link_peak = measure_h2d_peak(rig, min(1 << 30, max(1 << 20, cube_bytes)))
     cams = [cfg.camera(v) for v in range(cfg.n_views)]
     cam_structs = [vr.make_camera(c) for c in cams]
     samples_step = sum(W.nominal_samples(c, cfg.dims) for c in cams)
     tf = W.tf_haze(cfg.dims, cfg.step)
-    img = torch.empty((cfg.height, cfg.width, 4), dtype=torch.float32, device="cuda")
-    h_img = torch.empty((cfg.height, cfg.width, 4), dtype=torch.float32).pin_memory()
-    h_sum = torch.empty(32 + 8 * 256, dtype=torch.uint8).pin_memory()
+    img = rig.dev_empty((cfg.height, cfg.width, 4))
+    h_img = rig.host_empty((cfg.height, cfg.width, 4))
+    h_sum = rig.host_empty((32 + 8 * 256,), np.uint8)
     frame_ms, frame_h2d, sum_ms, sum_h2d = [], [], [], []
     last_range = [0.0, 1.0]
 
     def step(vol, out_img, record):
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 + len(cam_structs))]
-        ev[0].record(stream)
-        vol.minmax_histogram(256, out=h_sum)
+        ev = [rig.event() for _ in range(2 + len(cam_structs))]
+        rig.record(ev[0])
+        vol.minmax_histogram(256, out=h_sum, stream=rig.stream_arg)
         h2d_s = vol.stats()["h2d_bytes"]
-        ev[1].record(stream)
-        stream.synchronize()
-        hs = vr.Volume.read_summary(h_sum)
+        rig.record(ev[1])
+        rig.stream_synchronize()
+        hs = read_summary(rig, h_sum)
         last_range[0], last_range[1] = float(hs["vmin"]), float(hs["vmax"])
         vol.set_transfer_function(tf, last_range[0], last_range[1])
         h2d_f = []
         for k, c in enumerate(cam_structs):
-            vol.render(c, vr.VR_EA, out=out_img)
+            vol.render(c, vr.VR_EA, out=out_img, stream=rig.stream_arg)
             h2d_f.append(vol.stats()["h2d_bytes"])
-            ev[2 + k].record(stream)
-        stream.synchronize()
+            rig.record(ev[2 + k])
+        rig.stream_synchronize()
         if record:
-            sum_ms.append(ev[0].elapsed_time(ev[1])); sum_h2d.append(h2d_s)
+            sum_ms.append(rig.elapsed_ms(ev[0], ev[1])); sum_h2d.append(h2d_s)
             for k in range(len(cam_structs)):
-                frame_ms.append(ev[1 + k].elapsed_time(ev[2 + k])); frame_h2d.append(h2d_f[k])
+                frame_ms.append(rig.elapsed_ms(ev[1 + k], ev[2 + k])); frame_h2d.append(h2d_f[k])
         return h2d_s + sum(h2d_f)
 
     vol = vr.Volume(host, cfg.dims, brick=B, layout=vr.VR_BRICKED_HALO1, resident_bytes=resident,
                     n_copy_streams=cfg.n_copy_streams)
     for _ in range(args.warmup):
         step(vol, img, False)
-    torch.cuda.synchronize()
-    clocks = ClockSampler(physical_gpu_index(local)); clocks.start()
+    rig.synchronize()
+    clocks = rig.clock_sampler(); clocks.start()
     launches0 = vol.stats()["total_kernel_launches"]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
+    e0, e1 = rig.event(), rig.event()
+    rig.record(e0)
     h2d_step = 0
     for _ in range(args.steps):
         h2d_step = step(vol, img, True)
-    e1.record(stream); torch.cuda.synchronize()
+    rig.record(e1); rig.synchronize()
     clk = clocks.finish()
-    ms_step = e0.elapsed_time(e1) / args.steps
+    ms_step = rig.elapsed_ms(e0, e1) / args.steps
     launches = vol.stats()["total_kernel_launches"] - launches0
     vol.close()
 
     e2e_steps = max(1, min(args.steps, 2))
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record(stream)
+    a, b = rig.event(), rig.event()
+    rig.record(a)
     e2e_h2d = 0
     for _ in range(e2e_steps):
         with vr.Volume(host, cfg.dims, brick=B, layout=vr.VR_BRICKED_HALO1, resident_bytes=resident,
                        n_copy_streams=cfg.n_copy_streams) as hv:
             e2e_h2d = step(hv, h_img, False)
-    b.record(stream); torch.cuda.synchronize()
-    e2e_ms = a.elapsed_time(b) / e2e_steps
+    rig.record(b); rig.synchronize()
+    e2e_ms = rig.elapsed_ms(a, b) / e2e_steps
     ms_step, e2e_ms = max_over_ranks([ms_step, e2e_ms], dist, "cuda")
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
-        return
+        return None
     k_ms = float(np.mean(frame_ms))
     gbs = float(np.sum(frame_h2d)) / (float(np.sum(frame_ms)) * 1e-3) / 1e9
     sum_gbs = float(np.sum(sum_h2d)) / (float(np.sum(sum_ms)) * 1e-3) / 1e9
@@ -582,7 +662,8 @@ def run_ours_ooc(args, cfg):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": block, "clocks": clk,
             "e2e": {"value": world * samples_step / (e2e_ms * 1e-3), "unit": "samples/s",
-                    "h2d_bytes_per_step": int(e2e_h2d), "d2h_bytes_per_step": int(len(cams) * h_img.numel() * 4 + 32 + 8 * 256),
+                    "h2d_bytes_per_step": int(e2e_h2d),
+                    "d2h_bytes_per_step": int(len(cams) * cfg.height * cfg.width * 16 + 32 + 8 * 256),
                     "ms_per_step": e2e_ms, "steps": e2e_steps},
             "gpu_launches": int(launches),
             "roofline": {"bound": "host_link", "achieved": gbs, "peak": link_peak, "unit": "GB/s", "frac": gbs / link_peak,
@@ -601,7 +682,7 @@ def run_ours_ooc(args, cfg):
         cam = cfg.camera(0)
         mask = np.zeros((cam.height, cam.width), dtype=np.uint8)
         mask[4::8, 4::8] = 1
-        hn = host.numpy().reshape(-1, B + 1, B + 1, B + 1)
+        hn = rig.as_numpy(host).reshape(-1, B + 1, B + 1, B + 1)
         t0 = time.perf_counter()
         r = O.render(hn, cam, O.EA, tf, last_range[0], last_range[1], mask=mask, layout=O.BRICKED_HALO1,
                      layout_brick=B, dims=cfg.dims)
@@ -612,6 +693,7 @@ def run_ours_ooc(args, cfg):
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+    return line
 
 
 def main():

@@ -63,3 +63,108 @@ def test_ooc_config_cuts_whole_brick_layers():
 def test_config_block_names_the_workload():
     b = bench.config_block(W.get_config(2))
     assert "512x512x1024" in b["workload"] and b["cube_bytes"] == 1 << 30 and "model" not in b
+
+
+# ---------------------------------------------------------------------------------- the whole flow, emulated
+class _NoClocks:
+    def start(self):
+        pass
+
+    def finish(self):
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["emulated"]}
+
+
+class SimtRig:
+    """bench.TorchCudaRig's interface on the host emulation of the library (tests/simt): buffers are guarded host
+    allocations, "events" are host clock readings (the emulated runtime is synchronous)."""
+    name = "simt"
+    stream_arg = 0
+
+    def __init__(self):
+        sys.path.insert(0, os.path.join(ROOT, "tests", "simt"))
+        import simt_lib
+        self.lib = simt_lib
+
+    def host_empty(self, shape, dtype=np.float32, pinned=True):
+        return self.lib.Buffer(shape, dtype, device=False)
+
+    def dev_empty(self, shape, dtype=np.float32):
+        return self.lib.Buffer(shape, dtype, device=True)
+
+    def to_device(self, host):
+        return self.lib.Buffer.of(host.array, device=True)
+
+    def as_numpy(self, host):
+        return host.array
+
+    def read(self, t):
+        return np.array(t.array, copy=True)
+
+    def event(self):
+        return [0.0]
+
+    def record(self, e):
+        import time
+        e[0] = time.perf_counter()
+
+    def elapsed_ms(self, a, b):
+        return (b[0] - a[0]) * 1e3
+
+    def synchronize(self):
+        pass
+
+    stream_synchronize = empty_cache = synchronize
+
+    def copy_h2d(self, d, h):
+        d.array[...] = h.array
+
+    def clock_sampler(self):
+        return _NoClocks()
+
+
+def _args(**kw):
+    import argparse
+    d = dict(gpus=1, steps=1, warmup=1, impl="ours", config=2, no_cpu=False, no_e2e=False, cpu_seconds=0.3, ooc_nz=0,
+             ooc_resident_frac=0.25, path=0, lag=-1, no_zcopy=False, views=2)
+    d.update(kw)
+    return argparse.Namespace(**d)
+
+
+@pytest.mark.parametrize("number,scale", [(2, 1 / 16), (3, 1 / 32), (4, 1 / 64), (5, 1 / 32)])
+def test_bench_flow_and_json_line_in_emulation(number, scale, capsys):
+    """bench.py's own measurement flow — warm-up, timed steps, per-render events, cold cameras, the end-to-end leg with
+    host buffers, roofline arithmetic, cpu_baseline — executed on a scaled config against the emulated library: the
+    line the driver parses is assembled without an exception and carries every key of the contract."""
+    import json
+    rig = SimtRig()
+    cfg = W.get_config(number, scale=scale)
+    with rig.lib.emulated():
+        line = bench.run_ours(_args(config=number), rig=rig, cfg=cfg)
+    printed = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+    assert printed["metric"] == line["metric"] == "voxel_samples_per_s" and printed["unit"] == "samples/s"
+    for key in ("value", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline", "dtype",
+                "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert key in printed, key
+    assert printed["value"] > 0 and printed["gpu_launches"] > 0 and printed["dtype"] == "f32" and printed["vs_baseline"] is None
+    assert "workload" in printed["config"] and "model" not in printed["config"]
+    r = printed["roofline"]
+    assert r["bound"] in ("hbm", "alu", "host_link") and r["achieved"] > 0 and r["peak"] > 0 and "traffic" in r
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    e = printed["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] >= 4 * np.prod(cfg.dims) and e["d2h_bytes_per_step"] > 0
+    c = printed["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["value"] > 0 and c["cores"] >= 1 and "sample" in c
+    if number != 5:
+        assert printed["render_ms_cold"] is not None or cfg.sort_last
+        assert len(printed["render_ms_by_view"]) == 2 * len(cfg.modes)
+
+
+def test_reference_arm_line(capsys):
+    """--impl reference: the oracle on the host cores, same metric / unit / config block, the keys the contract adds."""
+    import json
+    line = bench.run_reference(_args(impl="reference", steps=2, warmup=1), cfg=W.get_config(4, scale=1 / 64))
+    printed = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+    assert printed == json.loads(json.dumps(line))
+    assert printed["impl"] == "reference" and printed["metric"] == "voxel_samples_per_s" and printed["value"] > 0
+    assert printed["cpu_baseline"]["kind"] == "oracle" and printed["cpu_baseline"]["value"] == printed["value"]
+    assert printed["e2e"] == {"value": printed["value"], "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
