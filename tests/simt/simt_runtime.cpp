@@ -254,6 +254,23 @@ void trace_corner_loads(bool active, const void *base, const void *p0, const voi
             }
             g_trace_stats[2] += 1; g_trace_stats[3] += (unsigned long long)nl; g_trace_stats[4] += (unsigned long long)ns;
         }
+        // what-if: ONE 16-byte load of the aligned quad that holds element p, plus a scalar load of p + 1 only for the
+        // lanes whose p is the last element of its quad (the alternative to two scalar loads per row)
+        for (int e = 0; e < 2; ++e) {
+            uint64_t lines[32];
+            int nl = 0, n_lanes = 0;
+            for (int l = 0; l < 32; ++l) {
+                if (!(t.present >> l & 1u) || t.v[l] == ~0ull) continue;
+                const bool last = ((t.v[l] >> 2) & 3u) == 3u;
+                if (e == 1 && !last) continue;
+                ++n_lanes;
+                const uint64_t ln = (e == 0 ? t.v[l] : t.v[l] + 4u) >> 7;
+                bool seen = false;
+                for (int k = 0; k < nl; ++k) seen = seen || lines[k] == ln;
+                if (!seen) lines[nl++] = ln;
+            }
+            if (n_lanes) { g_trace_stats[5] += 1; g_trace_stats[6] += (unsigned long long)nl; }
+        }
     }
 }
 

@@ -42,7 +42,7 @@ def run(cfg, v, cam, mode, variant):
             out = simt_lib.Buffer((cam.height, cam.width, 4) if mode == vr.VR_EA else (cam.height, cam.width))
             lib.simt_trace(1)
             vol.render(cam, mode, out=out, stream=0)
-            st = [lib.simt_trace_stat(i) for i in range(5)]
+            st = [lib.simt_trace_stat(i) for i in range(7)]
             lib.simt_trace(0)
     return st
 
@@ -63,26 +63,29 @@ def main():
           "lanes; lane efficiency = active lanes / (32 x warp iterations).  A fully coalesced load of 32 active lanes reads "
           "1-2 lines and 4-5 sectors.  Configs are scaled copies (volume and image by the same factor, so the pixel "
           "spacing in voxels — what decides coalescing — is the config's own).\n")
-    print("| config (scale) | view | variant | samples | lane efficiency | lines / load | sectors / load | sectors / active lane |")
-    print("|---|---|---|---:|---:|---:|---:|---:|")
+    print("`lines / sample` = 8 loads x lines per load / active lanes: the L1 cost of one sample.  `what-if 16 B` = the same with "
+          "ONE aligned 16-byte load per row (+ a scalar load for the lanes whose x is the last element of its quad) instead of "
+          "two scalar loads: a variant that is not built (DESIGN.md §10), counted here to size its gain.\n")
+    print("| config (scale) | view | variant | samples | lane efficiency | lines / load | sectors / load | lines / sample | what-if 16 B: lines / sample |")
+    print("|---|---|---|---:|---:|---:|---:|---:|---:|")
     for number in (int(x) for x in args.configs.split(",")):
         cfg = W.get_config(number, scale=SCALE[number])
         v = W.make_cube(cfg.recipe)
         mode = vr.VR_EA if "ea" in cfg.modes else vr.VR_MIP
         views = list(range(0, cfg.n_views, max(1, cfg.n_views // args.views)))[: args.views]
-        totals = {name: np.zeros(5) for name, _ in variants}
+        totals = {name: np.zeros(7) for name, _ in variants}
         for view in views:
             cam = cfg.camera(view).with_(flags=0)
             for name, var in variants:
                 st = np.array(run(cfg, v, cam, mode, var), dtype=np.float64)
                 totals[name] += st
-                it, act, ld, ln, sc = st
+                it, act, ld, ln, sc, qld, qln = st
                 print(f"| cfg{number} ({SCALE[number]:g}) | {view} | {name} | {int(act)} | {act / (32 * it):.2f} | {ln / ld:.2f} | "
-                      f"{sc / ld:.2f} | {sc / ld / (act / it):.3f} |")
+                      f"{sc / ld:.2f} | {ln / act:.2f} | {qln / act:.2f} |")
         for name, _ in variants:
-            it, act, ld, ln, sc = totals[name]
+            it, act, ld, ln, sc, qld, qln = totals[name]
             print(f"| **cfg{number} all views** | | **{name}** | {int(act)} | **{act / (32 * it):.2f}** | **{ln / ld:.2f}** | "
-                  f"**{sc / ld:.2f}** | {sc / ld / (act / it):.3f} |")
+                  f"**{sc / ld:.2f}** | **{ln / act:.2f}** | **{qln / act:.2f}** |")
 
 
 if __name__ == "__main__":
