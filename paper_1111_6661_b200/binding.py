@@ -18,7 +18,7 @@ VR_LINEAR, VR_BRICKED_HALO1 = 0, 1
 VR_DEVICE, VR_HOST_PINNED = 0, 1
 VR_EA, VR_MIP = 0, 1
 VR_SORT_LAST = 1
-VR_OPT_RENDER_PATH, VR_OPT_ZFAST_COPY, VR_OPT_LANE_LAG, VR_OPT_EMPTY_SKIP, VR_OPT_FORCE_WIDE = 1, 2, 3, 4, 5
+VR_OPT_RENDER_PATH, VR_OPT_ZFAST_COPY, VR_OPT_LANE_LAG, VR_OPT_EMPTY_SKIP, VR_OPT_FORCE_WIDE, VR_OPT_ROW_LOADS = 1, 2, 3, 4, 5, 6
 VR_PATH_AUTO, VR_PATH_RAY_MAJOR = 0, 1
 
 _STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_UNSUPPORTED", 3: "VR_ERR_OUT_OF_MEMORY",

@@ -176,8 +176,8 @@ struct PartK {
 
 // part != nullptr: write per-(ray, owner brick) fragments instead of pixels (no ERT, C.7)
 void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
-                 const MacroK &macro, const PartK *part, bool force_wide, int rows, float *image, long long pitch_f,
-                 cudaStream_t st);
+                 const MacroK &macro, const PartK *part, bool force_wide, bool quad_loads, int rows, float *image,
+                 long long pitch_f, cudaStream_t st);
 void launch_fragment_init(int mode, float *arena, unsigned long long n_frag, int grid, cudaStream_t st);
 void launch_transpose_xz(const float *in, float *out, int nx, int ny, int nz, cudaStream_t st);
 

@@ -82,15 +82,37 @@ __device__ __forceinline__ const float *cell_pointer(const LaneVolK &V, int ix, 
     return p;
 }
 
-template <bool WIDE, int FAST>
+// elements u and u + 1 of a row through ONE aligned 16-byte load of the quad that holds u (o = u & 3 is u's place in
+// it) plus, only where u ends its quad, a scalar load of u + 1.  Rows start 16-byte aligned and their length is a
+// multiple of 4 (checked by launch_rows), so the quad never leaves the row; u + 1 is a voxel by C.3.
+__device__ __forceinline__ void load_pair_quad(const float *quad, int o, float &a, float &b)
+{
+    const float4 q = __ldg(reinterpret_cast<const float4 *>(quad));
+    float e = 0.0f;
+    if (o == 3) e = __ldg(quad + 4);
+    const bool hi = (o & 2) != 0, odd = (o & 1) != 0;
+    const float t0 = hi ? q.z : q.x, t1 = hi ? q.w : q.y, t2 = hi ? e : q.z;
+    a = odd ? t1 : t0;
+    b = odd ? t2 : t1;
+}
+
+template <bool WIDE, int FAST, bool QUAD>
 __device__ __forceinline__ float sample_cell(const LaneVolK &V, int ix, int iy, int iz, float fx, float fy, float fz)
 {
-    const float *p = cell_pointer<WIDE, FAST>(V, ix, iy, iz);
+    const int o = QUAD ? ((FAST == 0 ? ix : iz) & 3) : 0;
+    // QUAD: p addresses the aligned quad of the fast index (the fast index enters the offset rounded down to 4)
+    const float *p = FAST == 0 ? cell_pointer<WIDE, FAST>(V, ix - o, iy, iz) : cell_pointer<WIDE, FAST>(V, ix, iy, iz - o);
     const float *pa = p + V.sa, *pb = p + V.sb, *pab = pb + V.sa;
-    const float q00 = __ldg(p), q01 = __ldg(p + 1);          // (a, b) = (0, 0): unit-stride neighbours
-    const float q10 = __ldg(pa), q11 = __ldg(pa + 1);        // a + 1
-    const float r00 = __ldg(pb), r01 = __ldg(pb + 1);        // b + 1
-    const float r10 = __ldg(pab), r11 = __ldg(pab + 1);      // a + 1, b + 1
+    float q00, q01, q10, q11, r00, r01, r10, r11;
+    if (QUAD) {
+        load_pair_quad(p, o, q00, q01); load_pair_quad(pa, o, q10, q11);
+        load_pair_quad(pb, o, r00, r01); load_pair_quad(pab, o, r10, r11);
+    } else {
+        q00 = __ldg(p); q01 = __ldg(p + 1);                  // (a, b) = (0, 0): unit-stride neighbours
+        q10 = __ldg(pa); q11 = __ldg(pa + 1);                // a + 1
+        r00 = __ldg(pb); r01 = __ldg(pb + 1);                // b + 1
+        r10 = __ldg(pab); r11 = __ldg(pab + 1);              // a + 1, b + 1
+    }
     // trilerp_packed(v000, v100, v010, v110, v001, v101, v011, v111): corner (X,Y,Z)
     if (FAST == 0)      // u = x, a = y, b = z
         return trilerp_packed(q00, q01, q10, q11, r00, r01, r10, r11, fx, fy, fz);
@@ -147,7 +169,7 @@ __device__ __forceinline__ void flush_fragment(const PartK &P, int cur, int i, i
 // PART: instead of one pixel value per ray, one fragment per (ray, owner brick): the ray state is flushed to the
 // brick's fragment and reset whenever the owner brick (ix/B, iy/B, iz/B) of the next sample changes — the same
 // samples in the same order as the per-brick marches of C.7, so the fragments are bit-identical to theirs.
-template <int MODE, bool ERT, bool WIDE, int FAST, bool SKIP, bool PART>
+template <int MODE, bool ERT, bool WIDE, int FAST, bool SKIP, bool PART, bool QUAD>
 __global__ void __launch_bounds__(kLaneThreads)
 k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__restrict__ image, long long pitch_f)
 {
@@ -219,7 +241,7 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__re
             unsigned int empty = 0u;
             if (SKIP && skipping) empty = __ldg(Mc.flag + ((iz >> 3) * cxy + (iy >> 3) * Mc.cx + (ix >> 3)));
             if (!SKIP || empty == 0u) {
-                const float s = sample_cell<WIDE, FAST>(V, ix, iy, iz, fx, fy, fz);
+                const float s = sample_cell<WIDE, FAST, QUAD>(V, ix, iy, iz, fx, fy, fz);
                 if (MODE == VR_MIP) m = fmaxf(m, s);
                 else {
                     composite_p(classify_s(tf_s, tf.scale, tf.bias, s), cr, cg, cb, T);
@@ -273,8 +295,8 @@ k_transpose_xz(const float *__restrict__ in, float *__restrict__ out, int nx, in
 }  // namespace
 
 void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
-                 const MacroK &macro, const PartK *part, bool force_wide, int rows, float *image, long long pitch_f,
-                 cudaStream_t st)
+                 const MacroK &macro, const PartK *part, bool force_wide, bool quad_loads, int rows, float *image,
+                 long long pitch_f, cudaStream_t st)
 {
     const int n_lane = map.lane_axis == 0 ? cam.width : cam.height;
     const dim3 g((unsigned)((n_lane + 31) / 32), (unsigned)((rows + kRowsPerCta - 1) / kRowsPerCta));
@@ -284,12 +306,16 @@ void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int f
                                     (unsigned long long)(fast == 0 ? vol.nx : vol.nz);
     const bool wide = force_wide || span > 0xffffffffull;
     const bool skip = mode == VR_EA && macro.flag != nullptr && !part;
+    // 16-byte row loads need rows that start 16-byte aligned (the base is, vr_create_volume) and hold a multiple of 4
+    const bool quad = quad_loads && !skip && !part && ((fast == 0 ? vol.nx : vol.nz) & 3) == 0 &&
+                      (((uintptr_t)vol.base) & 15u) == 0;
     PartK P;
     if (part) P = *part;
     else { P.bricks = nullptr; P.lut = nullptr; P.arena = nullptr; P.B = 1; P.nbx = P.nby = 0; }
-#define VR_L4(M, E, Wd, F, S) vr_launch(k_rows<M, E, Wd, F, S, false>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f)
+#define VR_L4(M, E, Wd, F, S) vr_launch(k_rows<M, E, Wd, F, S, false, false>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f)
 #define VR_L3(M, E, Wd, F) do { \
-        if (part) vr_launch(k_rows<M, false, Wd, F, false, true>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f); \
+        if (part) vr_launch(k_rows<M, false, Wd, F, false, true, false>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f); \
+        else if (quad) vr_launch(k_rows<M, E, Wd, F, false, false, true>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f); \
         else if (M == VR_EA && skip) VR_L4(M, E, Wd, F, (M == VR_EA)); else VR_L4(M, E, Wd, F, false); } while (0)
 #define VR_L2(M, E, Wd) do { if (fast == 0) VR_L3(M, E, Wd, 0); else VR_L3(M, E, Wd, 2); } while (0)
 #define VR_L1(M, E) do { if (wide) VR_L2(M, E, true); else VR_L2(M, E, false); } while (0)

@@ -65,19 +65,21 @@ def test_ray_caster_resources(sass, resources):
     transfer function is the only shared memory; 8 corner loads per sample (+ 1 byte of the skipping grid); packed
     FFMA2 lerps."""
     rows = {k: v for k, v in resources.items() if "k_rows<" in k}
-    assert len(rows) == 28                                            # MIP 4 + EA 8 + EA skip 8 + partials 8
+    assert len(rows) == 40                                            # MIP 4 + EA 8 + EA skip 8 + partials 8 + 16-byte loads 12
     for k, (reg, stack, shared, local) in rows.items():
         assert reg <= 48 and shared <= 5200, (k, reg, shared)
     for k, ops in sass.items():
         if "k_rows<" not in k:
             continue
         ldg = [op for op in ops if op.startswith("LDG")]
-        args = re.search(r"k_rows<(\d), (\w+), (\w+), (\d), (\w+), (\w+)>", k)
+        args = re.search(r"k_rows<(\d), (\w+), (\w+), (\d), (\w+), (\w+), (\w+)>", k)
         assert args, k
-        mode, ert, wide, fast, skip, part = (int(x) if x.isdigit() else x == "true" for x in args.groups())
+        mode, ert, wide, fast, skip, part, quad = (int(x) if x.isdigit() else x == "true" for x in args.groups())
         n_corner = len([op for op in ldg if ".U8" not in op and ".128" not in op and ".64" not in op])
         if part:                                                      # + the brick table reads of the two fragment flushes
             assert 8 <= n_corner <= 24, (k, ldg)
+        elif quad:                                                    # 4 quads + 4 predicated scalars (+ the staged table)
+            assert n_corner == 4 and len([op for op in ldg if ".128" in op]) >= 4, (k, ldg)
         else:
             assert n_corner == 8, (k, ldg)
         assert (len([op for op in ldg if ".U8" in op]) >= 1) == bool(skip), (k, ldg)

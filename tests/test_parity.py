@@ -449,6 +449,29 @@ def test_rays_along_brick_planes_and_opaque_first_sample(be):
         assert np.array_equal(g, o.image) and (g[o.K > 0] == 1.0).all()
 
 
+@pytest.mark.parametrize("n,wide", [((64, 44, 60), 0), ((64, 44, 60), 1), ((36, 40, 61), 0)])
+def test_16_byte_row_loads(be, n, wide):
+    """VR_OPT_ROW_LOADS = 1: one aligned 16-byte load per row (+ a scalar load where x ends its quad) instead of two
+    scalar loads — the same eight voxels, so bit-identical images; the memory-fast dimension must be a multiple of 4
+    (nz = 61: the z-fastest launches keep scalar loads, the x-fastest ones use quads); with and without 64-bit offsets."""
+    v = W.make_cube(W.Recipe(*n, seed=88, n_sources=6))
+    s = O.minmax_hist(v)
+    R = float(max(abs(s.vmin), abs(s.vmax)))
+    tf = W.tf_opaque(n, 0.5)
+    with vr.Volume(be.dev(v), n) as vol:
+        vol.set_option(vr.VR_OPT_ROW_LOADS, 1)
+        vol.set_option(vr.VR_OPT_FORCE_WIDE, wide)
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for name, cam in _axis_views(n, False):
+            for ert in (0.0, 0.99):
+                cam2 = cam.with_(ert_alpha=ert)
+                oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax)
+                assert np.array_equal(render(be, vol, cam2, vr.VR_EA), oe.image), (name, ert)
+            om = O.render(v, cam, O.MIP)
+            assert np.array_equal(render(be, vol, cam, vr.VR_MIP), om.image), name
+        assert vol.stats()["path"] == 7
+
+
 def test_mixed_camera_renders(be):
     """A camera whose origins AND directions vary per pixel (neither perspective nor orthographic)."""
     n = (32, 32, 32)
@@ -465,7 +488,7 @@ def test_set_option_rejects_bad_values(be):
     v = W.make_cube(W.Recipe(16, 16, 16, seed=1))
     with vr.Volume(be.dev(v), (16, 16, 16)) as vol:
         for opt, val in ((vr.VR_OPT_RENDER_PATH, 5), (vr.VR_OPT_ZFAST_COPY, 2), (vr.VR_OPT_LANE_LAG, -1),
-                         (vr.VR_OPT_EMPTY_SKIP, 2), (vr.VR_OPT_FORCE_WIDE, -1), (77, 0)):
+                         (vr.VR_OPT_EMPTY_SKIP, 2), (vr.VR_OPT_FORCE_WIDE, -1), (vr.VR_OPT_ROW_LOADS, 2), (77, 0)):
             with pytest.raises(vr.VrError) as e:
                 vol.set_option(opt, val)
             assert e.value.status == vr.VR_ERR_INVALID_ARG
