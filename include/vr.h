@@ -143,7 +143,10 @@ VR_API vr_status vr_set_transfer_function(vr_volume *vol, const float *rgba, flo
  *   VR_EA : channels = 4: premultiplied (C.r, C.g, C.b, 1-T); a miss is (0,0,0,0).
  *   VR_MIP: channels = 1: max of the interpolated samples in data units; no sample = -INFINITY.
  * Out-of-core volumes are rendered brick by brick in view order with the ray state carried in
- * the image (so ERT stays exact); uploads run on the copy streams and overlap rendering.
+ * the image (so ERT stays exact); uploads run on the copy streams and overlap rendering.  Once the
+ * value ranges gathered by the first vr_minmax_histogram of a brick-major volume have reached the
+ * host, an EA render drops every brick whose whole range maps to opacity exactly 0 before it is
+ * uploaded or marched (exact: such samples change nothing; VR_OPT_EMPTY_SKIP = 0 turns it off).
  * Errors: VR_ERR_INVALID_ARG (NULL, width/height 0, step <= 0 or non-finite, ert_alpha not in
  * [0,1), channels not matching mode, bad pitch), VR_ERR_NOT_READY (EA before a transfer
  * function was set), VR_ERR_UNSUPPORTED, VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA.
@@ -244,6 +247,9 @@ typedef struct {
     uint64_t resident_bytes;        /* device bytes owned by the handle */
     uint32_t zfast_copy;            /* 1: the handle holds a z-fastest copy of the volume (VR_OPT_ZFAST_COPY) */
     uint32_t skip_variant;          /* 1: the last render launched the empty-space-skipping kernel variant */
+    uint32_t bricks_empty;          /* bricks of a brick-major volume dropped by the last render because their whole value
+                                       range has opacity 0 (neither uploaded nor marched) */
+    uint32_t reserved;
     uint64_t macro_cells;           /* macrocells of the skipping grid (0: none built) */
     uint64_t empty_cells;           /* cells whose samples all have opacity 0 under the current transfer function,
                                        as of the last flag pass that has COMPLETED on its stream */

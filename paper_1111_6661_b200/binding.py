@@ -54,7 +54,8 @@ class vr_stats(C.Structure):
                 ("bricks_culled", C.c_uint32), ("path", C.c_uint32), ("kernel_launches", C.c_uint32),
                 ("fragments", C.c_uint64), ("h2d_bytes", C.c_uint64), ("d2h_bytes", C.c_uint64),
                 ("total_kernel_launches", C.c_uint64), ("resident_bytes", C.c_uint64),
-                ("zfast_copy", C.c_uint32), ("skip_variant", C.c_uint32), ("macro_cells", C.c_uint64),
+                ("zfast_copy", C.c_uint32), ("skip_variant", C.c_uint32), ("bricks_empty", C.c_uint32),
+                ("reserved", C.c_uint32), ("macro_cells", C.c_uint64),
                 ("empty_cells", C.c_uint64)]
 
 

@@ -4,6 +4,7 @@
 // vr_reduce.cu.  No host synchronisation on the in-HBM paths; everything is enqueued on the
 // caller's stream, library copy streams are joined to it by events.
 #include <algorithm>
+#include <cfloat>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -103,6 +104,13 @@ struct vr_volume {
     int mc[3] = { 0, 0, 0 };
     int opt_skip = 1;
 
+    // value range of every brick slot of a brick-major volume, gathered by the first summary pass (device, pinned
+    // host copy, event recorded after the copy): lets the chain and sort-last paths drop bricks whose samples all
+    // have opacity 0 BEFORE they are uploaded or marched (S38)
+    BrickRangeK *d_brick_rng = nullptr, *h_brick_rng = nullptr;
+    cudaEvent_t brick_rng_ev = nullptr;
+    bool brick_rng_issued = false;
+
     // scratch
     SummaryScratch *d_sum = nullptr;
     vr_summary *d_sum_out = nullptr;          // staging for host outputs
@@ -148,6 +156,9 @@ static void free_volume(vr_volume *v)
     if (v->macro_flag) cudaFree(v->macro_flag);
     if (v->d_nskip) cudaFree(v->d_nskip);
     if (v->h_nskip) cudaFreeHost(v->h_nskip);
+    if (v->d_brick_rng) cudaFree(v->d_brick_rng);
+    if (v->h_brick_rng) cudaFreeHost(v->h_brick_rng);
+    if (v->brick_rng_ev) cudaEventDestroy(v->brick_rng_ev);
     if (v->zfast_ev) cudaEventDestroy(v->zfast_ev);
     v->arena.release();
     v->host_image.release();
@@ -317,6 +328,52 @@ static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam,
                               const PartK *part, float *img, long long pitch_f, cudaStream_t st);
 static bool lanes_addressable(const vr_volume *v);
 
+// ------------------------------------------------------------------ empty bricks (S38)
+// C.4 table index of a scalar, the float32 sequence of classify() (host code is built without contraction)
+static inline int tf_index_host(float s, float scale, float bias)
+{
+    float u = fmaf(s, scale, bias);
+    u = u != u ? 0.0f : fminf(fmaxf(u, 0.0f), 1.0f);
+    const int i = (int)(u * 255.0f);
+    return i > 254 ? 254 : i;
+}
+
+// every sample that reads only voxels of [mn, mx] has opacity exactly 0 under the handle's transfer function
+// (same argument and same dilation as k_macro_flags, vr_macro.cu)
+static bool range_is_empty(const vr_volume *v, float mn, float mx)
+{
+    if (!(mn >= -FLT_MAX && mx <= FLT_MAX && mn <= mx)) return false;
+    const float e = fmaf(fmaxf(fabsf(mn), fabsf(mx)), 4.76837158203125e-7f, FLT_MIN);
+    const int lo = tf_index_host(mn - e, v->tf_scale, v->tf_bias), hi = tf_index_host(mx + e, v->tf_scale, v->tf_bias);
+    for (int j = lo; j <= hi + 1; ++j)
+        if (v->tf_tab[4 * j + 3] != 0.0f) return false;
+    return true;
+}
+
+static inline float key_to_float(unsigned int k)
+{
+    const unsigned int b = (k & 0x80000000u) ? (k & 0x7fffffffu) : ~k;
+    float f; memcpy(&f, &b, 4); return f;
+}
+
+// drops the bricks of a brick-major volume whose slot range maps to opacity 0 (EA only; needs the ranges of the
+// first summary pass to have ARRIVED on the host: no waiting here)
+static void cull_empty_bricks(vr_volume *v, int mode, std::vector<PlannedBrick> &plan)
+{
+    v->stats.bricks_empty = 0;
+    if (mode != VR_EA || !v->opt_skip || !v->tf_has_zero || !v->brick_rng_issued) return;
+    if (cudaEventQuery(v->brick_rng_ev) != cudaSuccess) { cudaGetLastError(); return; }
+    size_t keep = 0;
+    for (size_t i = 0; i < plan.size(); ++i) {
+        const BrickRangeK &r = v->h_brick_rng[plan[i].id];
+        const bool empty = !r.bad && range_is_empty(v, key_to_float(r.enc_min), key_to_float(r.enc_max));
+        if (empty) { v->stats.bricks_empty++; continue; }
+        if (keep != i) plan[keep] = plan[i];
+        ++keep;
+    }
+    plan.resize(keep);
+}
+
 // Sort-last (C.7, A10): per-(pixel, brick) fragments over each brick's screen rectangle, folded per pixel in
 // visibility order by k_composite.  Fragments of a VR_LINEAR volume come from ONE lane-mapped march per frame
 // that flushes the ray state at every change of owner brick; bricks of a resident VR_BRICKED_HALO1 volume are
@@ -327,6 +384,7 @@ static vr_status render_sort_last(vr_volume *v, const vr_camera *c, const CamK &
     std::vector<PlannedBrick> plan;
     uint32_t culled = 0;
     plan_bricks(v, c, plan, culled);
+    cull_empty_bricks(v, mode, plan);
     const int W = cam.width, H = cam.height;
     const int bins_x = (W + 15) / 16, bins_y = (H + 15) / 16;
     // fragments, work items, bins
@@ -426,6 +484,7 @@ static vr_status render_chain(vr_volume *v, const vr_camera *c, const CamK &cam,
     std::vector<PlannedBrick> plan;
     uint32_t culled = 0;
     plan_bricks(v, c, plan, culled);
+    cull_empty_bricks(v, mode, plan);
     VolK V;
     V.nx = (int)v->desc.nx; V.ny = (int)v->desc.ny; V.nz = (int)v->desc.nz;
     V.base = nullptr; V.sy = V.sz = 0; V.ox = V.oy = V.oz = 0;
@@ -621,7 +680,7 @@ static vr_status sweep_volume(vr_volume *v, cudaStream_t st, int grid, Flat &&fl
                 for (int a = 0; a < 3; ++a) ext[a] = (int)std::min(v->B, n[a] - bb[a] * v->B);   // halo excluded
                 box.ex = ext[0]; box.ey = ext[1]; box.ez = ext[2];
                 const int bgrid = (int)std::max<long long>(1, std::min<long long>(grid, ((long long)box.ey * box.ez + 15) / 16));
-                box_fn(box, bgrid);
+                box_fn(box, bgrid, id);
                 v->stats.kernel_launches += 1;
                 if (v->out_of_core) { vr_status rc = stream_brick_release(v, slot, st); if (rc != VR_OK) return rc; }
             }
@@ -792,7 +851,7 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     VR_CUDA(cudaSetDevice(v->device));
     cudaStream_t st = (cudaStream_t)stream;
     v->stats.kernel_launches = 0; v->stats.h2d_bytes = 0; v->stats.d2h_bytes = 0; v->stats.fragments = 0;
-    v->stats.bricks_drawn = v->stats.bricks_culled = 0;
+    v->stats.bricks_drawn = v->stats.bricks_culled = v->stats.bricks_empty = 0;
 
     float *img = im->pixels;
     long long pitch_f = (long long)(pitch / 4);
@@ -845,6 +904,19 @@ VR_API vr_status vr_minmax_histogram(vr_volume *v, uint32_t nbins, const float *
     launch_summary_reset(S, st);
     v->stats.kernel_launches += 1;
     const int n_pass = range ? 1 : 2;
+    // brick-major volumes: the first summary call also gathers the value range of every brick slot (the data is
+    // immutable while the handle exists), which later renders use to drop empty bricks before upload
+    bool gather_ranges = false;
+    if (v->desc.layout == VR_BRICKED_HALO1 && !v->brick_rng_issued) {
+        if (!v->d_brick_rng) {
+            VR_CUDA(cudaMalloc(&v->d_brick_rng, v->n_bricks * sizeof(BrickRangeK)));
+            VR_CUDA(cudaMallocHost(&v->h_brick_rng, v->n_bricks * sizeof(BrickRangeK)));
+            VR_CUDA(cudaEventCreateWithFlags(&v->brick_rng_ev, cudaEventDisableTiming));
+        }
+        launch_brick_range_init(v->d_brick_rng, v->n_bricks, st);
+        v->stats.kernel_launches += 1;
+        gather_ranges = true;
+    }
     for (int pass = 0; pass < n_pass; ++pass) {
         // pass 0: min/max (+ histogram when the caller gave the range); pass 1: histogram over [min,max]
         if (range && pass == 0) { launch_summary_range(S, 1, lo, hi, nbins, st); v->stats.kernel_launches += 1; }
@@ -855,12 +927,22 @@ VR_API vr_status vr_minmax_histogram(vr_volume *v, uint32_t nbins, const float *
                 else if (range) launch_minmax_hist_flat(p, n, nbins, S, g, st);
                 else launch_minmax_flat(p, n, S, g, st);
             },
-            [&](const BoxK &box, int g) {
+            [&](const BoxK &box, int g, uint64_t id) {
                 if (pass == 1) launch_hist_box(box, nbins, S, g, st);
                 else if (range) launch_minmax_hist_box(box, nbins, S, g, st);
                 else launch_minmax_box(box, S, g, st);
+                if (gather_ranges && pass == 0) {        // the whole slot, halo included: what the brick's samples read
+                    launch_brick_range(box.base, v->brick_elems, v->d_brick_rng + id, std::max(1, std::min(g, 64)), st);
+                    v->stats.kernel_launches += 1;
+                }
             });
         if (rc != VR_OK) return rc;
+        if (gather_ranges && pass == 0) {
+            VR_CUDA(cudaMemcpyAsync(v->h_brick_rng, v->d_brick_rng, v->n_bricks * sizeof(BrickRangeK), cudaMemcpyDeviceToHost, st));
+            VR_CUDA(cudaEventRecord(v->brick_rng_ev, st));
+            v->brick_rng_issued = true;
+            v->stats.d2h_bytes += v->n_bricks * sizeof(BrickRangeK);
+        }
     }
     if (out_location == VR_DEVICE) launch_summary_finish(S, nbins, out, st);
     else {
@@ -898,7 +980,7 @@ VR_API vr_status vr_statistics(vr_volume *v, vr_statistics_result *out, uint32_t
     for (int pass = 0; pass < 5; ++pass) {
         rc = sweep_volume(v, st, grid,
             [&](const float *p, unsigned long long n, int g) { launch_stat_pass_flat(pass, p, n, S, g, st); },
-            [&](const BoxK &box, int g) { launch_stat_pass_box(pass, box, S, g, st); });
+            [&](const BoxK &box, int g, uint64_t) { launch_stat_pass_box(pass, box, S, g, st); });
         if (rc != VR_OK) return rc;
         launch_stat_step(S, pass, st);
         v->stats.kernel_launches += 1;

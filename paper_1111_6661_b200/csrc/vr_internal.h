@@ -165,6 +165,11 @@ void launch_macro_flags(const float2 *mm, long long n_cells, const TfK &tf, unsi
                         int grid, cudaStream_t st);
 void launch_macro_blocks(unsigned char *flag, const MacroK &m, int grid, cudaStream_t st);
 
+// value range of a brick slot as order-preserving keys (key(f) = bits ^ (sign ? ~0 : 0x80000000)); bad: non-finite seen
+struct BrickRangeK { unsigned int enc_min, enc_max, bad, pad; };
+void launch_brick_range_init(BrickRangeK *r, unsigned long long n, cudaStream_t st);
+void launch_brick_range(const float *v, unsigned long long n, BrickRangeK *r, int grid, cudaStream_t st);
+
 // sort-last partials written by the lane-mapped kernel: plan-ordered brick table, brick-grid -> plan index (-1:
 // culled), fragment arena, brick edge and grid
 struct PartK {

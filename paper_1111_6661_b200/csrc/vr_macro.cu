@@ -112,7 +112,44 @@ __global__ void __launch_bounds__(256) k_macro_blocks(unsigned char *__restrict_
     }
 }
 
+// value range of one brick slot (all (B+1)^3 voxels a sample owned by the brick can read): order-preserving keys
+// of min and max over the finite voxels, and whether a non-finite voxel was seen.  r is zero-initialised to
+// { key(+inf), key(-inf), 0 } by k_brick_range_init.
+__global__ void __launch_bounds__(256) k_brick_range_init(BrickRangeK *r, unsigned long long n)
+{
+    const unsigned long long i = (unsigned long long)blockIdx.x * 256 + threadIdx.x;
+    if (i < n) { r[i].enc_min = 0xff800000u; r[i].enc_max = 0x007fffffu; r[i].bad = 0u; r[i].pad = 0u; }
+}
+
+__global__ void __launch_bounds__(256) k_brick_range(const float *__restrict__ v, unsigned long long n, BrickRangeK *r)
+{
+    unsigned int kmin = 0xffffffffu, kmax = 0u, bad = 0u;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * 256) {
+        const float a = __ldg(v + i);
+        if (fabsf(a) <= FLT_MAX) {
+            const unsigned int b = __float_as_uint(a), k = (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+            kmin = min(kmin, k); kmax = max(kmax, k);
+        } else bad = 1u;
+    }
+    kmin = __reduce_min_sync(0xffffffffu, kmin); kmax = __reduce_max_sync(0xffffffffu, kmax);
+    bad = __reduce_or_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0) {
+        atomicMin(&r->enc_min, kmin); atomicMax(&r->enc_max, kmax);
+        if (bad) atomicOr(&r->bad, 1u);
+    }
+}
+
 }  // namespace
+
+void launch_brick_range_init(BrickRangeK *r, unsigned long long n, cudaStream_t st)
+{
+    vr_launch(k_brick_range_init, (unsigned)((n + 255) / 256), 256, 0, st, r, n);
+}
+
+void launch_brick_range(const float *v, unsigned long long n, BrickRangeK *r, int grid, cudaStream_t st)
+{
+    vr_launch(k_brick_range, grid, 256, 0, st, v, n, r);
+}
 
 void launch_macro_blocks(unsigned char *flag, const MacroK &m, int grid, cudaStream_t st)
 {

@@ -86,6 +86,7 @@ cudaError_t cudaEventCreateWithFlags(cudaEvent_t *e, unsigned int flags);
 cudaError_t cudaEventDestroy(cudaEvent_t e);
 cudaError_t cudaEventRecord(cudaEvent_t e, cudaStream_t s);
 cudaError_t cudaEventSynchronize(cudaEvent_t e);
+cudaError_t cudaEventQuery(cudaEvent_t e);
 cudaError_t cudaGetDevice(int *d);
 cudaError_t cudaSetDevice(int d);
 cudaError_t cudaDeviceGetAttribute(int *v, cudaDeviceAttr a, int dev);

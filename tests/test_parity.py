@@ -588,6 +588,56 @@ def test_bricked_halo_chain_and_streaming(be, where):
             assert st["h2d_bytes"] > 0 and st["resident_bytes"] == 11 * brick_bytes
 
 
+@pytest.mark.parametrize("where", ["device", "host_ooc"])
+def test_empty_bricks_are_dropped_before_upload(be, where):
+    """A brick-major cube that is transparent under TF_SOURCES except around one blob: after the first summary pass
+    has gathered the value range of every brick slot, an EA render drops the empty bricks — out of core they are not
+    even uploaded — and the image is still bit-identical to the oracle (S38).  MIP never drops a brick."""
+    n, B = (60, 44, 52), 12
+    nx, ny, nz = n
+    rng = np.random.default_rng(23)
+    v = (-1.0 + 0.05 * rng.standard_normal((nz, ny, nx))).astype(np.float32)
+    z, y, x = np.mgrid[0:nz, 0:ny, 0:nx]
+    v += (12.0 * np.exp(-((x - 40.0) ** 2 + (y - 30.0) ** 2 + (z - 12.0) ** 2) / (2 * 4.0 ** 2))).astype(np.float32)
+    v[0, 0, 0] = np.nan                                             # a brick with a non-finite voxel is never dropped
+    t = W.retile_halo(v, B)
+    s = O.minmax_hist(v)
+    tf = W.tf_sources(n, 0.5, alpha_scale=6.0)
+    brick_bytes = (B + 1) ** 3 * 4
+    kw = dict(resident_bytes=10 * brick_bytes, n_copy_streams=3) if where == "host_ooc" else {}
+    data = be.dev(t) if where == "device" else be.pinned(t)
+    cams = [c for _, c in _views(n)]
+    with vr.Volume(data, n, brick=B, layout=vr.VR_BRICKED_HALO1, **kw) as vol:
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        g0 = render(be, vol, cams[0], vr.VR_EA)                      # before any summary pass: nothing is known, nothing dropped
+        st0 = vol.stats()
+        assert st0["bricks_empty"] == 0
+        assert_summary_equal(summary(be, vol), s)                    # gathers the brick ranges
+        be.sync()
+        for cam in cams:
+            for ert in (0.0, 0.99):
+                cam2 = cam.with_(ert_alpha=ert)
+                oe = O.render(v, cam2, O.EA, tf, s.vmin, s.vmax)
+                g = render(be, vol, cam2, vr.VR_EA)
+                assert np.array_equal(g, oe.image, equal_nan=True)
+                st = vol.stats()
+                assert st["bricks_empty"] > 0.5 * st["n_bricks"] and st["bricks_drawn"] + st["bricks_empty"] + st["bricks_culled"] == st["n_bricks"]
+            om = O.render(v, cam, O.MIP)
+            assert np.array_equal(render(be, vol, cam, vr.VR_MIP), om.image) and vol.stats()["bricks_empty"] == 0
+        assert np.array_equal(g0, O.render(v, cams[0], O.EA, tf, s.vmin, s.vmax).image, equal_nan=True)
+        if where == "host_ooc":
+            render(be, vol, cams[0], vr.VR_EA)
+            assert vol.stats()["h2d_bytes"] < 0.5 * st0["h2d_bytes"]  # most of the streamed bricks were not uploaded
+        # sort-last on the resident brick-major volume drops them too
+        if where == "device":
+            sl = cams[0].with_(flags=W.cameras.VR_SORT_LAST)
+            ob = O.render(v, sl, O.EA, tf, s.vmin, s.vmax, brick=B)
+            assert np.array_equal(render(be, vol, sl, vr.VR_EA), ob.image, equal_nan=True) and vol.stats()["bricks_empty"] > 0
+        vol.set_option(vr.VR_OPT_EMPTY_SKIP, 0)
+        render(be, vol, cams[0], vr.VR_EA)
+        assert vol.stats()["bricks_empty"] == 0
+
+
 def test_host_linear_mirror_and_host_outputs(be):
     n = (40, 36, 52)
     v = W.make_cube(W.Recipe(*n, seed=37, n_sources=3))
