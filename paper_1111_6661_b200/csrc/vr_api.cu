@@ -100,6 +100,7 @@ struct vr_volume {
     float2 *macro_mm = nullptr;
     unsigned char *macro_flag = nullptr;
     unsigned long long *d_nskip = nullptr, *h_nskip = nullptr;
+    cudaEvent_t nskip_ev = nullptr;           // recorded after the count of empty cells was copied to h_nskip
     bool macro_failed = false, macro_flags_dirty = true;
     int mc[3] = { 0, 0, 0 };
     int opt_skip = 1;
@@ -156,6 +157,7 @@ static void free_volume(vr_volume *v)
     if (v->macro_flag) cudaFree(v->macro_flag);
     if (v->d_nskip) cudaFree(v->d_nskip);
     if (v->h_nskip) cudaFreeHost(v->h_nskip);
+    if (v->nskip_ev) cudaEventDestroy(v->nskip_ev);
     if (v->d_brick_rng) cudaFree(v->d_brick_rng);
     if (v->h_brick_rng) cudaFreeHost(v->h_brick_rng);
     if (v->brick_rng_ev) cudaEventDestroy(v->brick_rng_ev);
@@ -572,6 +574,7 @@ static vr_status ensure_macro(vr_volume *v, const TfK &tf, cudaStream_t st, Macr
         v->macro_mm = mm; v->macro_flag = fl;
         VR_CUDA(cudaMalloc(&v->d_nskip, sizeof(unsigned long long)));
         VR_CUDA(cudaMallocHost(&v->h_nskip, sizeof(unsigned long long)));
+        VR_CUDA(cudaEventCreateWithFlags(&v->nskip_ev, cudaEventDisableTiming));
         *v->h_nskip = 0;
         MacroK G; G.flag = nullptr; G.n_skip = nullptr; G.min_skip = 0; G.cx = v->mc[0]; G.cy = v->mc[1]; G.cz = v->mc[2];
         launch_macro_minmax(v->dev_data, n[0], n[1], n[2], G, v->macro_mm, st);
@@ -585,13 +588,19 @@ static vr_status ensure_macro(vr_volume *v, const TfK &tf, cudaStream_t st, Macr
         launch_macro_flags(v->macro_mm, cells, tf, v->macro_flag, v->d_nskip,
                            (int)std::min<long long>((cells + 255) / 256, (long long)v->sm_count * 8), st);
         VR_CUDA(cudaMemcpyAsync(v->h_nskip, v->d_nskip, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        VR_CUDA(cudaEventRecord(v->nskip_ev, st));
         MacroK G; G.flag = nullptr; G.n_skip = nullptr; G.min_skip = 0; G.cx = v->mc[0]; G.cy = v->mc[1]; G.cz = v->mc[2];
         launch_macro_blocks(v->macro_flag, G, (int)std::min<long long>((cells / 512 + 8) / 8, (long long)v->sm_count * 8), st);
         v->stats.kernel_launches += 2;
         v->macro_flags_dirty = false;
     }
+    const unsigned long long min_skip = (unsigned long long)std::max<long long>(1, cells / 64);   // worth a byte load per sample from ~1.6 % empty cells
+    // once the count of this transfer function has reached the host (no waiting), a grid with too few empty cells
+    // is not consulted at all: the plain kernel variant is launched
+    if (cudaEventQuery(v->nskip_ev) == cudaSuccess) { if (*v->h_nskip < min_skip) return VR_OK; }
+    else cudaGetLastError();
     M.flag = v->macro_flag; M.n_skip = v->d_nskip;
-    M.min_skip = (unsigned long long)std::max<long long>(1, cells / 64);      // worth a byte load per sample from ~1.6 % empty cells
+    M.min_skip = min_skip;
     M.cx = v->mc[0]; M.cy = v->mc[1]; M.cz = v->mc[2];
     v->stats.skip_variant = 1;
     v->stats.macro_cells = (uint64_t)cells;
@@ -803,12 +812,15 @@ VR_API vr_status vr_set_transfer_function(vr_volume *v, const float *rgba, float
     bool has_zero = false;
     for (int i = 0; i < 1024; ++i)
         VR_REQUIRE(std::isfinite(rgba[i]) && rgba[i] >= 0.0f && rgba[i] <= 1.0f, "table entry %d = %g is outside [0,1]", i, rgba[i]);
+    const float scale = 1.0f / (vmax - vmin), bias = -vmin * scale;   // C.4, float32
+    if (v->tf_set && scale == v->tf_scale && bias == v->tf_bias && memcmp(v->tf_tab, rgba, 1024 * sizeof(float)) == 0)
+        return VR_OK;                                               // the same table and range again: nothing to redo
     for (int i = 0; i < 1024; ++i) v->tf_tab[i] = rgba[i];
     for (int c = 0; c < 4; ++c) v->tf_tab[1024 + c] = rgba[1020 + c];      // pad entry (never weighted: i <= 254)
     for (int i = 0; i < 255; ++i) has_zero = has_zero || (rgba[4 * i + 3] == 0.0f && rgba[4 * i + 7] == 0.0f);
     v->tf_has_zero = has_zero;                                       // some table interval has opacity exactly 0
-    v->tf_scale = 1.0f / (vmax - vmin);                             // C.4, float32
-    v->tf_bias = -vmin * v->tf_scale;
+    v->tf_scale = scale;
+    v->tf_bias = bias;
     v->tf_dirty = true;                                             // uploaded on the stream of the next render
     v->macro_flags_dirty = true;
     v->tf_set = true;

@@ -290,14 +290,17 @@ def test_empty_space_skipping_is_exact(be, n):
         oe = O.render(v, cam, O.EA, tf2, s.vmin, s.vmax)
         assert np.array_equal(render(be, vol, cam, vr.VR_EA), oe.image, equal_nan=True)
         assert vol.stats()["skip_variant"] == 0
-        # TF_HAZE has an empty interval but no cell of a noise cube falls into it: the variant is launched and
-        # decides on the device not to skip
+        # TF_HAZE has an empty interval but no cell of a noise cube falls into it: either the skipping variant is
+        # launched and decides on the device not to skip (the count has not reached the host yet), or the host already
+        # knows and launches the plain variant (always so in the emulation, whose runtime is synchronous)
         tf3 = W.tf_haze(n, 0.5)
         vol.set_transfer_function(tf3, s.vmin, s.vmax)
         oe = O.render(v, cam, O.EA, tf3, s.vmin, s.vmax)
         assert np.array_equal(render(be, vol, cam, vr.VR_EA), oe.image, equal_nan=True)
         be.sync()
-        assert vol.stats()["skip_variant"] == 1 and vol.stats()["empty_cells"] < max(1, vol.stats()["macro_cells"] // 64)
+        assert vol.stats()["empty_cells"] < max(1, vol.stats()["macro_cells"] // 64)
+        assert np.array_equal(render(be, vol, cam, vr.VR_EA), oe.image, equal_nan=True)
+        assert vol.stats()["skip_variant"] == 0                      # by now the host knows: plain variant
         vol.set_option(vr.VR_OPT_EMPTY_SKIP, 0)
         vol.set_transfer_function(tf, s.vmin, s.vmax)
         oe = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
