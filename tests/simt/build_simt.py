@@ -10,7 +10,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_1111_6661_b200", "csrc")
-LIB = os.path.join(HERE, "libvr_simt.so")
+UBSAN = bool(os.environ.get("VR_SIMT_UBSAN"))
+LIB = os.path.join(HERE, "libvr_simt_ubsan.so" if UBSAN else "libvr_simt.so")
 
 
 def sources():
@@ -31,6 +32,9 @@ def build(force: bool = False) -> str:
         objs = []
         flags = ["-std=c++17", "-O2", "-g", "-fPIC", "-fvisibility=hidden", "-mfma", "-ffp-contract=off",
                  "-fno-strict-aliasing", "-Wall", "-Wno-unknown-pragmas", "-Wno-unused-function"]
+        if UBSAN:                                # VR_SIMT_UBSAN=1: abort on out-of-bounds indices of fixed-size (shared-
+            flags += ["-fsanitize=bounds,shift,integer-divide-by-zero,signed-integer-overflow,null,alignment",   # memory)
+                      "-fno-sanitize-recover=all"]       # arrays, misaligned vector accesses, signed overflow, bad shifts
         cmd = ["g++"] + flags + ["-shared", "-o", LIB]
         for s in sources():
             cmd += ["-x", "c++", "-include", os.path.join(HERE, "simt_host.h"), s]
