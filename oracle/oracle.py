@@ -198,3 +198,22 @@ def statistics(vol: np.ndarray, layout: int = LINEAR, layout_brick: int = 0, dim
     if rc != 0:
         raise ValueError(f"oracle_statistics failed: {rc}")
     return Statistics(int(st.n_finite), int(st.n_nonfinite), float(st.mean), float(st.stddev), np.float32(st.median))
+
+
+def encode_rgba8(image: np.ndarray, mode: int, background=(0.0, 0.0, 0.0), vmin: float = 0.0, vmax: float = 1.0) -> np.ndarray:
+    """C.14 (S40): 8-bit RGBA frame of an EA image (H,W,4) composited over an opaque background, or of a MIP image
+    (H,W) as a grey ramp over [vmin, vmax]."""
+    lib = _load()
+    img = np.ascontiguousarray(image, dtype=np.float32)
+    H, W = img.shape[:2]
+    assert img.shape == ((H, W, 4) if mode == EA else (H, W))
+    bg = np.asarray(background, dtype=np.float32)
+    out = np.empty((H, W, 4), dtype=np.uint8)
+    lib.oracle_encode_rgba8.restype = C.c_int
+    lib.oracle_encode_rgba8.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint64, C.c_int, C.c_void_p, C.c_float,
+                                        C.c_float, C.c_void_p]
+    rc = lib.oracle_encode_rgba8(img.ctypes.data, W, H, W * (4 if mode == EA else 1), mode, bg.ctypes.data,
+                                 float(vmin), float(vmax), out.ctypes.data)
+    if rc != 0:
+        raise ValueError(f"oracle_encode_rgba8 failed: {rc}")
+    return out

@@ -570,6 +570,42 @@ ORACLE_EXPORT int oracle_statistics(const float *vol, uint32_t nx, uint32_t ny, 
     return 0;
 }
 
+/* ------------------------------------------------------------------ */
+/* C.14: 8-bit frame for delivery to a thin client                     */
+/* (the headless "service" side of PAPER.md:L48, L70; reading S40)     */
+/* ------------------------------------------------------------------ */
+/* EA image (premultiplied C, opacity A): the frame is composited over an opaque constant background,
+ * x_c = fmaf(1 - A, bg_c, C_c), clamped to [0,1] (NaN -> 0), byte = round-half-even(x_c * 255); alpha byte 255.
+ * MIP image (scalar m, miss = -inf): grey ramp u = sat(fmaf(m, scale, bias)) with scale = 1/(vmax - vmin),
+ * bias = -vmin * scale (as C.4), byte = round-half-even(u * 255) in r, g, b; alpha byte 255.
+ * img: [H][W][4] or [H][W] floats with a row pitch in floats; out: [H][W][4] bytes, tightly packed. */
+static inline uint8_t byte_of_unit(float x)
+{
+    x = x != x ? 0.0f : fminf(fmaxf(x, 0.0f), 1.0f);
+    return (uint8_t)lrintf(x * 255.0f);              /* default rounding mode: to nearest, ties to even */
+}
+
+ORACLE_EXPORT int oracle_encode_rgba8(const float *img, uint32_t W, uint32_t H, uint64_t pitch_f, int mode,
+                                      const float bg[3], float vmin, float vmax, uint8_t *out)
+{
+    if (!img || !out || !W || !H) return -1;
+    const float scale = 1.0f / (vmax - vmin), bias = -vmin * scale;
+    for (uint32_t j = 0; j < H; ++j)
+        for (uint32_t i = 0; i < W; ++i) {
+            uint8_t *o = out + 4 * ((size_t)j * W + i);
+            if (mode == ORACLE_EA) {
+                const float *p = img + (size_t)j * pitch_f + 4 * (size_t)i;
+                const float w = 1.0f - p[3];
+                for (int c = 0; c < 3; ++c) o[c] = byte_of_unit(fmaf(w, bg[c], p[c]));
+            } else {
+                const uint8_t g = byte_of_unit(fmaf(img[(size_t)j * pitch_f + i], scale, bias));
+                o[0] = o[1] = o[2] = g;
+            }
+            o[3] = 255;
+        }
+    return 0;
+}
+
 ORACLE_EXPORT int oracle_num_threads(void)
 {
     int n = 1;

@@ -520,3 +520,40 @@ def test_p16_statistics_bricked_halo_layout_equals_linear():
     a, b = O.statistics(v), O.statistics(t, layout=O.BRICKED_HALO1, layout_brick=8, dims=(21, 18, 26))
     assert a.n_finite == b.n_finite and a.median == b.median
     assert abs(a.mean - b.mean) < 1e-14 and abs(a.stddev - b.stddev) < 1e-14      # same values, another voxel order
+
+
+# --------------------------------------------------------------------------- P17: 8-bit frame for delivery (C.14, S40)
+def test_p17_encode_closed_forms():
+    """Opaque pixels of colour k/255 give byte k for every k; transparent pixels give the background; the tie 127.5 goes
+    to the even byte 128; values outside [0,1] clamp; NaN gives 0; the alpha byte is 255.  MIP: grey ramp, miss = 0."""
+    k = np.arange(256, dtype=np.float64)
+    img = np.zeros((1, 256, 4), dtype=np.float32)
+    img[0, :, 0] = (k / 255).astype(np.float32); img[0, :, 1] = ((255 - k) / 255).astype(np.float32); img[0, :, 3] = 1.0
+    out = O.encode_rgba8(img, O.EA, background=(0.3, 0.6, 0.9))
+    assert np.array_equal(out[0, :, 0], np.arange(256)) and np.array_equal(out[0, :, 1], 255 - np.arange(256))
+    assert (out[0, :, 2] == 0).all() and (out[..., 3] == 255).all()
+    clear = np.zeros((2, 3, 4), dtype=np.float32)
+    out = O.encode_rgba8(clear, O.EA, background=(0.5, 0.2, 1.0))
+    assert (out[..., 0] == 128).all() and (out[..., 1] == 51).all() and (out[..., 2] == 255).all()     # 127.5 -> 128 (even)
+    half = np.zeros((1, 1, 4), dtype=np.float32); half[0, 0] = (0.25, 2.0, -1.0, 0.5)       # C + (1 - A) bg
+    out = O.encode_rgba8(half, O.EA, background=(0.5, 0.5, 0.5))
+    assert tuple(out[0, 0]) == (128, 255, 0, 255)                                           # 0.5 -> 127.5 -> 128; clamps
+    bad = np.zeros((1, 1, 4), dtype=np.float32); bad[0, 0] = (np.nan, np.inf, -np.inf, 0.0)
+    assert tuple(O.encode_rgba8(bad, O.EA)[0, 0]) == (0, 255, 0, 255)
+    m = np.array([[-np.inf, 2.0, 3.0, 4.0, 10.0, np.nan]], dtype=np.float32)
+    out = O.encode_rgba8(m, O.MIP, vmin=2.0, vmax=4.0)
+    assert out[0, :, 0].tolist() == [0, 0, 128, 255, 255, 0] and np.array_equal(out[..., 0], out[..., 1]) and (out[..., 3] == 255).all()
+
+
+def test_p17_encode_against_float64():
+    """A random EA image against the formula evaluated in float64: equal bytes wherever the float64 value is not
+    within 1e-4 of a rounding tie, never more than one byte apart elsewhere."""
+    img = RNG.random((37, 53, 4)).astype(np.float32)
+    img[..., :3] *= img[..., 3:4]                                                         # premultiplied
+    bg = np.array([0.1, 0.7, 0.35], dtype=np.float32)
+    out = O.encode_rgba8(img, O.EA, background=bg).astype(np.int64)
+    x = np.clip(img[..., :3].astype(np.float64) + (1.0 - img[..., 3:4].astype(np.float64)) * bg.astype(np.float64), 0, 1) * 255
+    want = np.rint(x).astype(np.int64)
+    near_tie = np.abs(x - np.floor(x) - 0.5) < 1e-4
+    assert np.array_equal(out[..., :3][~near_tie], want[~near_tie]) and np.abs(out[..., :3] - want).max() <= 1
+    assert near_tie.mean() < 0.01
