@@ -230,6 +230,34 @@ typedef struct {
 VR_API vr_status vr_statistics(vr_volume *vol, vr_statistics_result *out, uint32_t out_location, void *stream);
 
 /* ------------------------------------------------------------------------------------------
+ * vr_encode_rgba8 — the 8-bit frame a thin client displays ("remote
+ * ... viewer ... is only responsible for ... result display", L70; reading S40 / C.14).  No graphics API
+ * is involved: the frame is a byte buffer.
+ *   src        a rendered image of this library: DEVICE float32, VR_EA (4 channels, premultiplied C and
+ *              opacity A) or VR_MIP (1 channel); src->row_pitch_bytes as in vr_render.
+ *   VR_EA      x_c = fmaf(1 - A, background_c, C_c), clamped to [0,1] (NaN -> 0);
+ *              byte_c = round-half-even(x_c * 255); alpha byte 255.
+ *   VR_MIP     u = sat(fmaf(m, scale, bias)) with scale = 1/(vmax - vmin), bias = -vmin * scale (float32, as
+ *              C.4); byte = round-half-even(u * 255) in r, g and b; a miss (-INFINITY) gives 0; alpha 255.
+ *   out        width*height RGBA8 pixels, rows of out_pitch_bytes (>= 4*width, multiple of 4; 0 = tight), DEVICE
+ *              (out_location VR_DEVICE) or pinned HOST (VR_HOST_PINNED: encoded into an internal device buffer
+ *              and copied on `stream`), 4-byte aligned.
+ * Enqueued on `stream` after whatever produced `src` there.
+ * Errors: VR_ERR_INVALID_ARG (NULL, bad sizes / mode / pitch, non-finite background, vmax <= vmin for VR_MIP),
+ * VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+    uint32_t struct_size;
+    uint32_t width, height;
+    uint32_t mode;               /* VR_EA or VR_MIP: what `src` holds */
+    float background[3];         /* VR_EA: opaque background colour, each in [0,1] */
+    float vmin, vmax;            /* VR_MIP: scalar range of the grey ramp */
+} vr_encode_desc;
+
+VR_API vr_status vr_encode_rgba8(vr_volume *vol, const vr_encode_desc *desc, const vr_image *src, uint8_t *out,
+                                 uint64_t out_pitch_bytes, uint32_t out_location, void *stream);
+
+/* ------------------------------------------------------------------------------------------
  * vr_get_stats — counters of the last vr_render / vr_minmax_histogram on this handle
  * (SURVEY.md §5 "metrics"): host-side values only, no synchronisation.
  * ------------------------------------------------------------------------------------------ */

@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvr.so")
-SOURCES = ["vr_api.cu", "vr_reduce.cu", "vr_stats.cu", "vr_raycast.cu", "vr_lanes.cu", "vr_macro.cu"]
+SOURCES = ["vr_api.cu", "vr_reduce.cu", "vr_stats.cu", "vr_raycast.cu", "vr_lanes.cu", "vr_macro.cu", "vr_encode.cu"]
 HEADERS = ["vr_internal.h", "vr_plan.h", "vr_math.cuh", "vr_range.cuh", "vr_sweep.cuh", "vr_lanemap.h", os.path.join("..", "..", "include", "vr.h")]
 
 NVCC_FLAGS = [

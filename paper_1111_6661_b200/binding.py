@@ -64,8 +64,13 @@ class vr_statistics_result(C.Structure):
                 ("median", C.c_float), ("reserved", C.c_uint32)]
 
 
+class vr_encode_desc(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("width", C.c_uint32), ("height", C.c_uint32), ("mode", C.c_uint32),
+                ("background", C.c_float * 3), ("vmin", C.c_float), ("vmax", C.c_float)]
+
+
 EXPORTS = ("vr_create_volume", "vr_destroy_volume", "vr_set_transfer_function", "vr_render",
-           "vr_minmax_histogram", "vr_statistics", "vr_get_stats", "vr_set_option", "vr_last_error", "vr_version")
+           "vr_minmax_histogram", "vr_statistics", "vr_encode_rgba8", "vr_get_stats", "vr_set_option", "vr_last_error", "vr_version")
 
 _lib = None
 
@@ -89,6 +94,9 @@ def _declare(lib):
         lib.vr_minmax_histogram.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
         lib.vr_statistics.restype = C.c_int
         lib.vr_statistics.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+        lib.vr_encode_rgba8.restype = C.c_int
+        lib.vr_encode_rgba8.argtypes = [C.c_void_p, C.POINTER(vr_encode_desc), C.POINTER(vr_image), C.c_void_p,
+                                        C.c_uint64, C.c_uint32, C.c_void_p]
         lib.vr_get_stats.restype = C.c_int
         lib.vr_get_stats.argtypes = [C.c_void_p, C.POINTER(vr_stats)]
         lib.vr_set_option.restype = C.c_int
@@ -256,6 +264,26 @@ class Volume:
             torch.cuda.current_stream().synchronize()
             buf = buf.cpu()
         return np.frombuffer(buf.numpy().tobytes()[: C.sizeof(vr_statistics_result)], dtype=STATISTICS_DTYPE)[0]
+
+    # -- vr_encode_rgba8
+    def encode_rgba8(self, image, mode: int, out, background=(0.0, 0.0, 0.0), vmin: float = 0.0, vmax: float = 1.0,
+                     stream=None):
+        """Enqueue the 8-bit frame of a rendered device image.  `out`: uint8 tensor (H,W,4), CUDA or pinned CPU."""
+        H, W = int(image.shape[0]), int(image.shape[1])
+        d = vr_encode_desc()
+        d.struct_size = C.sizeof(vr_encode_desc)
+        d.width, d.height, d.mode = W, H, int(mode)
+        d.background = (C.c_float * 3)(*[float(x) for x in background])
+        d.vmin, d.vmax = float(vmin), float(vmax)
+        im = vr_image()
+        im.struct_size = C.sizeof(vr_image)
+        im.channels = 4 if mode == VR_EA else 1
+        im.location = VR_DEVICE
+        im.pixels = image.data_ptr()
+        im.row_pitch_bytes = image.stride(0) * 4
+        _check(load().vr_encode_rgba8(self._h, C.byref(d), C.byref(im), out.data_ptr(), out.stride(0),
+                                      VR_DEVICE if out.is_cuda else VR_HOST_PINNED, _stream_ptr(stream)))
+        return out
 
     # -- vr_set_option
     def set_option(self, option: int, value: int):

@@ -118,6 +118,7 @@ struct vr_volume {
     StatScratch *d_stat = nullptr;            // vr_statistics (allocated on first use)
     vr_statistics_result *d_stat_out = nullptr;
     DevBuf<float> arena, host_image;
+    DevBuf<unsigned int> host_frame;          // vr_encode_rgba8 with a pinned-host output
 
     // lane-mapped path: the library's z-fastest copy of a resident linear volume (vr_lanes.cu)
     float *zfast = nullptr;
@@ -164,6 +165,7 @@ static void free_volume(vr_volume *v)
     if (v->zfast_ev) cudaEventDestroy(v->zfast_ev);
     v->arena.release();
     v->host_image.release();
+    v->host_frame.release();
     delete v;
 }
 
@@ -1006,6 +1008,58 @@ VR_API vr_status vr_statistics(vr_volume *v, vr_statistics_result *out, uint32_t
     v->stats.kernel_launches += 1;
     VR_CUDA(cudaGetLastError());
     v->stats.total_kernel_launches += v->stats.kernel_launches;
+    return VR_OK;
+}
+
+VR_API vr_status vr_encode_rgba8(vr_volume *v, const vr_encode_desc *d, const vr_image *src, uint8_t *out,
+                                 uint64_t out_pitch_bytes, uint32_t out_location, void *stream)
+{
+    g_err[0] = 0;
+    VR_REQUIRE(v && d && src && out, "vr_encode_rgba8: NULL argument");
+    VR_REQUIRE(d->struct_size == sizeof(vr_encode_desc), "vr_encode_desc.struct_size %u != %zu", d->struct_size, sizeof(vr_encode_desc));
+    VR_REQUIRE(src->struct_size == sizeof(vr_image), "vr_image.struct_size %u != %zu", src->struct_size, sizeof(vr_image));
+    VR_REQUIRE(d->mode == VR_EA || d->mode == VR_MIP, "bad mode %u", d->mode);
+    VR_REQUIRE(d->width > 0 && d->height > 0 && d->width <= 65536 && d->height <= 65536, "bad image size %ux%u", d->width, d->height);
+    const uint32_t ch = d->mode == VR_EA ? 4u : 1u;
+    VR_REQUIRE(src->channels == ch && src->location == VR_DEVICE && src->pixels, "src must be a DEVICE image of %u channel(s)", ch);
+    const uint64_t row_bytes = (uint64_t)d->width * ch * 4;
+    const uint64_t pitch = src->row_pitch_bytes ? src->row_pitch_bytes : row_bytes;
+    VR_REQUIRE(pitch >= row_bytes && pitch % (d->mode == VR_EA ? 16 : 4) == 0, "bad src row_pitch_bytes %llu", (unsigned long long)pitch);
+    VR_REQUIRE(((uintptr_t)src->pixels & (d->mode == VR_EA ? 15u : 3u)) == 0, "src pixels are misaligned");
+    const uint64_t out_row = (uint64_t)d->width * 4;
+    const uint64_t opitch = out_pitch_bytes ? out_pitch_bytes : out_row;
+    VR_REQUIRE(opitch >= out_row && opitch % 4 == 0 && ((uintptr_t)out & 3u) == 0, "bad out pitch / alignment");
+    VR_REQUIRE(out_location == VR_DEVICE || out_location == VR_HOST_PINNED, "bad out_location %u", out_location);
+    EncodeK P;
+    P.scale = P.bias = 0.0f;
+    for (int c = 0; c < 3; ++c) {
+        P.bg[c] = d->background[c];
+        VR_REQUIRE(d->mode != VR_EA || (std::isfinite(P.bg[c]) && P.bg[c] >= 0.0f && P.bg[c] <= 1.0f), "background must be in [0,1]");
+    }
+    if (d->mode == VR_MIP) {
+        VR_REQUIRE(std::isfinite(d->vmin) && std::isfinite(d->vmax) && d->vmax > d->vmin, "need finite vmin < vmax (got %g, %g)", d->vmin, d->vmax);
+        P.scale = 1.0f / (d->vmax - d->vmin);                       // C.4 / C.14, float32
+        P.bias = -d->vmin * P.scale;
+    }
+    VR_CUDA(cudaSetDevice(v->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    v->stats.kernel_launches = 0; v->stats.h2d_bytes = 0; v->stats.d2h_bytes = 0;
+    unsigned int *dst = reinterpret_cast<unsigned int *>(out);
+    long long dst_pitch_w = (long long)(opitch / 4);
+    if (out_location == VR_HOST_PINNED) {
+        vr_status rc = v->host_frame.reserve((size_t)d->width * d->height);
+        if (rc != VR_OK) return rc;
+        dst = v->host_frame.p; dst_pitch_w = d->width;
+    }
+    launch_encode_rgba8((int)d->mode, src->pixels, (long long)(pitch / 4), (int)d->width, (int)d->height, P, dst, dst_pitch_w, st);
+    v->stats.kernel_launches = 1;
+    VR_CUDA(cudaGetLastError());
+    if (out_location == VR_HOST_PINNED) {
+        if (opitch == out_row) VR_CUDA(cudaMemcpyAsync(out, dst, out_row * d->height, cudaMemcpyDeviceToHost, st));
+        else VR_CUDA(cudaMemcpy2DAsync(out, opitch, dst, out_row, out_row, d->height, cudaMemcpyDeviceToHost, st));
+        v->stats.d2h_bytes = out_row * d->height;
+    }
+    v->stats.total_kernel_launches += 1;
     return VR_OK;
 }
 

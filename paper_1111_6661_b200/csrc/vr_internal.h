@@ -139,6 +139,11 @@ void launch_chain_brick(int mode, bool ert, bool force_wide, const CamK &cam, co
                         const BrickK &brick, float *image, long long pitch_f, cudaStream_t st);
 void launch_chain_finish(int W, int H, float *image, long long pitch_f, cudaStream_t st);
 
+// ---------------------------------------------------------------- 8-bit frame for delivery (vr_encode.cu)
+struct EncodeK { float bg[3]; float scale, bias; };
+void launch_encode_rgba8(int mode, const float *img, long long pitch_f, int W, int H, const EncodeK &P, unsigned int *out,
+                         long long out_pitch_w, cudaStream_t st);
+
 // ---------------------------------------------------------------- lane-mapped ray casting (vr_lanes.cu)
 // A resident volume as the kernel addresses it: one axis has element stride 1 (`fast`: 0 = the caller's
 // x-fastest array, 2 = the library's z-fastest copy); sa, sb are the element strides of the other two

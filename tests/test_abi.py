@@ -21,7 +21,8 @@ def declared_functions():
 
 def test_header_declares_the_north_star_calls():
     names = declared_functions()
-    for n in ("vr_create_volume", "vr_set_transfer_function", "vr_render", "vr_minmax_histogram"):
+    for n in ("vr_create_volume", "vr_set_transfer_function", "vr_render", "vr_minmax_histogram", "vr_statistics",
+              "vr_encode_rgba8"):
         assert n in names
     assert sorted(binding.EXPORTS) == names
 

@@ -857,6 +857,40 @@ def test_cfg5_scaled_out_of_core():
     del host
 
 
+# ------------------------------------------------------------------ §8(f) #4: the 8-bit frame a thin client displays
+def test_encode_rgba8_matches_oracle(be):
+    """vr_encode_rgba8 of rendered EA and MIP images (device and pinned-host outputs, a padded output pitch), byte for
+    byte against the oracle's C.14; plus a synthetic image with ties, out-of-range values and NaN."""
+    n = (40, 36, 52)
+    v = W.make_cube(W.Recipe(*n, seed=61, n_sources=3))
+    s = O.minmax_hist(v)
+    tf = W.tf_opaque(n, 0.5)
+    cam = W.orbit_camera(n, 1, 8, 90, 61, step=0.5, ert_alpha=0.99)
+    bg = (0.1, 0.25, 0.8)
+    with vr.Volume(be.dev(v), n) as vol:
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        ea_buf = be.empty((61, 90, 4)); vol.render(cam, vr.VR_EA, out=ea_buf, stream=be.stream)
+        mip_buf = be.empty((61, 90)); vol.render(cam, vr.VR_MIP, out=mip_buf, stream=be.stream)
+        ea, mip = be.numpy(ea_buf), be.numpy(mip_buf)
+        for device in (True, False):
+            out = be.empty((61, 90, 4), np.uint8, device=device)
+            vol.encode_rgba8(ea_buf, vr.VR_EA, out, background=bg, stream=be.stream)
+            assert np.array_equal(be.numpy(out), O.encode_rgba8(ea, O.EA, background=bg))
+            vol.encode_rgba8(mip_buf, vr.VR_MIP, out, vmin=float(s.vmin), vmax=float(s.vmax), stream=be.stream)
+            assert np.array_equal(be.numpy(out), O.encode_rgba8(mip, O.MIP, vmin=s.vmin, vmax=s.vmax))
+        syn = np.random.default_rng(5).random((33, 47, 4)).astype(np.float32) * 1.4 - 0.2
+        syn[0, 0] = (np.nan, np.inf, -np.inf, 0.5); syn[1, :, :3] = 0.5; syn[1, :, 3] = 1.0; syn[2] = 0.0
+        sb = be.dev(syn)
+        out = be.empty((33, 47, 4), np.uint8)
+        vol.encode_rgba8(sb, vr.VR_EA, out, background=(0.5, 0.5, 0.5), stream=be.stream)
+        g = be.numpy(out)
+        assert np.array_equal(g, O.encode_rgba8(syn, O.EA, background=(0.5, 0.5, 0.5)))
+        assert (g[1, :, :3] == 128).all() and (g[2, :, :3] == 128).all() and (g[..., 3] == 255).all()
+        with pytest.raises(vr.VrError) as e:
+            vol.encode_rgba8(sb, vr.VR_EA, out, background=(0.5, 2.0, 0.5), stream=be.stream)
+        assert e.value.status == vr.VR_ERR_INVALID_ARG
+
+
 # ------------------------------------------------------------------ S24: non-finite voxels in a rendered cube
 def test_nonfinite_voxels_render_like_the_oracle(be):
     """FITS blanks: NaN and +-Inf voxels.  A NaN sample classifies as table entry 0 and is ignored by MIP (C.4, C.6,
