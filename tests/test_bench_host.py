@@ -138,6 +138,9 @@ def test_bench_flow_and_json_line_in_emulation(number, scale, capsys):
     import json
     rig = SimtRig()
     cfg = W.get_config(number, scale=scale)
+    if number == 5:                                     # 48 bricks instead of cfg5's 3072: one emulated launch per brick
+        from dataclasses import replace
+        cfg = replace(cfg, brick=32, recipe=replace(cfg.recipe, nx=128, ny=128, nz=96), name="cfg5-test")
     with rig.lib.emulated():
         line = bench.run_ours(_args(config=number), rig=rig, cfg=cfg)
     printed = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
