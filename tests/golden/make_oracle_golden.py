@@ -30,11 +30,13 @@ def case():
     ea = O.render(v, cam, O.EA, tf, s.vmin, s.vmax)
     mip = O.render(v, cam, O.MIP)
     eab = O.render(v, cam.with_(ert_alpha=0.0), O.EA, tf, s.vmin, s.vmax, brick=4)
-    return v, s, ea, mip, eab
+    st = O.statistics(v)
+    frame = O.encode_rgba8(ea.image, O.EA, background=(0.1, 0.2, 0.3))
+    return v, s, ea, mip, eab, st, frame
 
 
 def lines():
-    v, s, ea, mip, eab = case()
+    v, s, ea, mip, eab, st, frame = case()
     yield "# written by tests/golden/make_oracle_golden.py (oracle only); float32 bit patterns in hex"
     yield "cube_checksum %016x" % W.checksum(v)
     yield "minmax %08x %08x" % (np.float32(s.vmin).view(np.uint32), np.float32(s.vmax).view(np.uint32))
@@ -44,6 +46,9 @@ def lines():
     yield "ea_ert " + " ".join("%08x" % x for x in ea.image.view(np.uint32).ravel())
     yield "mip " + " ".join("%08x" % x for x in mip.image.view(np.uint32).ravel())
     yield "ea_bricked4 " + " ".join("%08x" % x for x in eab.image.view(np.uint32).ravel())
+    yield "statistics %d %d %016x %016x %08x" % (st.n_finite, st.n_nonfinite, np.float64(st.mean).view(np.uint64),
+                                                 np.float64(st.stddev).view(np.uint64), np.float32(st.median).view(np.uint32))
+    yield "frame_rgba8 " + " ".join("%02x" % x for x in frame.ravel())
 
 
 if __name__ == "__main__":
