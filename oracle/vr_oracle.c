@@ -486,8 +486,9 @@ ORACLE_EXPORT int oracle_minmax_hist(const float *vol, uint32_t nx, uint32_t ny,
                 if (v < lo) { ++n_below; continue; }
                 if (v > hi) { ++n_above; continue; }
                 float t = (v - lo) * scale_h;
-                int64_t b = (int64_t)t;
-                if (b >= (int64_t)nbins) b = nbins - 1;
+                /* S41: a range so narrow or so wide that the bin arithmetic overflows gives t = +inf or NaN
+                 * (inf * 0); the conversion is then DEFINED as: NaN -> bin 0, t >= nbins -> last bin */
+                int64_t b = t != t ? 0 : t >= (float)nbins ? (int64_t)nbins - 1 : (int64_t)t;
                 counts[b]++;
             }
     head->n_below = n_below; head->n_above = n_above;

@@ -245,10 +245,12 @@ inline float __fdiv_rn(float a, float b) { return a / b; }
 inline float __fsqrt_rn(float a) { return sqrtf(a); }
 inline float __fdividef(float a, float b) { return a / b; }      // approximate on hardware; only used for estimates
 inline float __saturatef(float a) { return a != a ? 0.0f : fminf(fmaxf(a, 0.0f), 1.0f); }
-inline int __float2int_rd(float a) { return (int)floorf(a); }
-inline int __float2int_rz(float a) { return (int)a; }
-inline int __float2int_rn(float a) { return (int)nearbyintf(a); }
-inline int __float2int_ru(float a) { return (int)ceilf(a); }
+// cvt.r?i.s32.f32 saturates and turns NaN into 0 (a C cast is undefined there)
+inline int simt_cvt_s32(float r) { return r != r ? 0 : r >= 2147483648.0f ? 2147483647 : r <= -2147483648.0f ? (-2147483647 - 1) : (int)r; }
+inline int __float2int_rd(float a) { return simt_cvt_s32(floorf(a)); }
+inline int __float2int_rz(float a) { return simt_cvt_s32(truncf(a)); }
+inline int __float2int_rn(float a) { return simt_cvt_s32(nearbyintf(a)); }
+inline int __float2int_ru(float a) { return simt_cvt_s32(ceilf(a)); }
 inline unsigned int __float_as_uint(float f) { unsigned int u; memcpy(&u, &f, 4); return u; }
 inline float __uint_as_float(unsigned int u) { float f; memcpy(&f, &u, 4); return f; }
 inline int __float_as_int(float f) { int u; memcpy(&u, &f, 4); return u; }

@@ -557,3 +557,14 @@ def test_p17_encode_against_float64():
     near_tie = np.abs(x - np.floor(x) - 0.5) < 1e-4
     assert np.array_equal(out[..., :3][~near_tie], want[~near_tie]) and np.abs(out[..., :3] - want).max() <= 1
     assert near_tie.mean() < 0.01
+
+
+def test_p4_histogram_ranges_that_overflow_the_bin_arithmetic():
+    """S41.  A caller range of the whole float32 span: hi - lo = inf, scale_h = 0, every t is 0 or inf * 0 = NaN -> bin 0.
+    A range narrower than nbins / FLT_MAX: scale_h = inf, v == lo gives NaN -> bin 0, v > lo gives inf -> last bin."""
+    v = np.array([-3.0e38, 3.0e38, 0.0, 1.0, -1.0, 2.5, 1e-40, 7.0], dtype=np.float32).reshape(2, 2, 2)
+    s = O.minmax_hist(v, 16, (-3.4e38, 3.4e38))
+    assert s.counts[0] == 8 and s.counts[1:].sum() == 0 and s.n_below == s.n_above == 0
+    w = np.array([0.0, 1e-40, 5e-41, 0.0, 1e-40, -1.0, 1.0, 1e-40], dtype=np.float32).reshape(2, 2, 2)
+    s = O.minmax_hist(w, 16, (0.0, 1e-40))
+    assert s.counts[0] == 2 and s.counts[15] == 4 and s.n_below == 1 and s.n_above == 1 and s.counts.sum() == 6

@@ -50,6 +50,16 @@ def test_minmax_hist_nonfinite_and_constant(be):
         assert np.all(g["counts"] == k.size // 256)
 
 
+def test_histogram_ranges_that_overflow_the_bin_arithmetic(be):
+    """S41: caller ranges whose bin arithmetic overflows (scale_h = 0 with an infinite v - lo, or scale_h = inf): NaN goes
+    to bin 0 and +inf to the last bin on both sides (the float-to-int conversion of the GPU, made explicit in the oracle)."""
+    v = np.array([-3.0e38, 3.0e38, 0.0, 1.0, -1.0, 2.5, 1e-40, 7.0], dtype=np.float32).reshape(2, 2, 2)
+    w = np.array([0.0, 1e-40, 5e-41, 0.0, 1e-40, -1.0, 1.0, 1e-40], dtype=np.float32).reshape(2, 2, 2)
+    for a, rng in ((v, (-3.4e38, 3.4e38)), (w, (0.0, 1e-40)), (v, (-3.0e38, 3.0e38))):
+        with vr.Volume(be.dev(a), (2, 2, 2)) as vol:
+            assert_summary_equal(summary(be, vol, 16, rng), O.minmax_hist(a, 16, rng))
+
+
 # ------------------------------------------------------------------ §8(f) #1: mean, standard deviation, median
 def assert_statistics_equal(g, o, v):
     """Counts and the median (a data value) bit-exact; the float64 moments within 1e-13 of the data scale: both
