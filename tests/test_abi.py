@@ -104,3 +104,38 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in text.lower().replace("no cpu fallback", ""), f
+
+
+def test_c_client_compiles_and_links_against_the_library(tmp_path):
+    """A plain C translation unit that uses every entry point of include/vr.h the way README.md shows compiles with
+    -Wall -Werror and links against libvr.so (C linkage, no CUDA or C++ types in the interface); it is not run."""
+    src = tmp_path / "client.c"
+    src.write_text(r'''
+#include "vr.h"
+#include <stddef.h>
+int client(const float *dev_voxels, float *dev_img, vr_summary *sum_dev, unsigned char *frame, void *stream,
+           const float *tf, vr_statistics_result *st)
+{
+    vr_volume_desc d = { sizeof d, 64, 64, 64, 16, VR_LINEAR, VR_DEVICE, 0, dev_voxels, 0 };
+    vr_volume *vol = NULL;
+    if (vr_create_volume(&d, &vol) != VR_OK) return 1;
+    vr_minmax_histogram(vol, 256, NULL, sum_dev, VR_DEVICE, stream);
+    vr_set_transfer_function(vol, tf, -1.0f, 1.0f);
+    vr_camera cam = { sizeof cam, 32, 32, {0, 0, -1}, {2, 0, 0}, {0, 2, 0}, {0, 0, 1}, {0, 0, 0}, {0, 0, 0}, 1.0f, 0.99f, 0 };
+    vr_image img = { sizeof img, 4, VR_DEVICE, 0, dev_img, 0 };
+    vr_render(vol, &cam, VR_EA, &img, stream);
+    vr_encode_desc e = { sizeof e, 32, 32, VR_EA, {0, 0, 0}, 0, 0 };
+    vr_encode_rgba8(vol, &e, &img, frame, 0, VR_HOST_PINNED, stream);
+    vr_statistics(vol, st, VR_HOST_PINNED, stream);
+    vr_set_option(vol, VR_OPT_EMPTY_SKIP, 1);
+    vr_stats s = { sizeof s };
+    vr_get_stats(vol, &s);
+    return vr_destroy_volume(vol) == VR_OK && vr_last_error()[0] == 0 && vr_version() != NULL ? 0 : 2;
+}
+int main(void) { return 0; }
+''')
+    exe = tmp_path / "client"
+    lib = vr.library_path()
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-Wno-missing-field-initializers", "-I", os.path.join(ROOT, "include"),
+                    str(src), "-o", str(exe), "-L", os.path.dirname(lib), "-l:" + os.path.basename(lib),
+                    "-Wl,-rpath," + os.path.dirname(lib)], check=True)
