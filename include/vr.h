@@ -1,13 +1,15 @@
 /*
  * vr.h — C ABI of libvr.so: B200-native bricked volume ray-casting of float32 spectral
- * cubes plus the min/max + histogram summary passes.
+ * cubes plus the data passes the paper names: min/max + histogram, mean / standard deviation /
+ * median, and the 8-bit frame a thin client displays.
  *
  * What is computed.  The paper names the operations — interactive volume rendering of
  * larger-than-memory spectral cubes by sub-cube partitioning and a gather of partial images
  * and the "simple data analysis tasks" minimum/maximum
- * and histogram — but gives no formulae.  The arithmetic is therefore the
- * set of readings C.0-C.8 of SURVEY.md §8(c), restated in DESIGN.md §3.  Every entry point
- * below cites the passage and the reading it implements.
+ * and histogram, the "global view" tasks median and standard deviation (L66),
+ * a viewer that only displays results (L48, L70) — but gives no formulae.  The arithmetic is
+ * therefore the set of readings C.0-C.8 of SURVEY.md §8(c) and C.13-C.14, S33-S41 of DESIGN.md §3.
+ * Every entry point below cites the passage and the reading it implements.
  *
  * Conventions common to all calls
  *   - Plain C, no CUDA or torch types: a stream is passed as `void*` holding a cudaStream_t
@@ -15,11 +17,13 @@
  *   - Every call returns vr_status; nothing throws, aborts or prints.  vr_last_error() gives a
  *     thread-local message for the last failing call on this thread.
  *   - Every struct starts with `struct_size` = sizeof(that struct) as the caller compiled it.
- *   - vr_render / vr_minmax_histogram ENQUEUE work on `stream` and return; results are valid
- *     once `stream` reaches the point after the call.  With device-resident volumes and
+ *   - vr_render / vr_minmax_histogram / vr_statistics / vr_encode_rgba8 ENQUEUE work on `stream` and
+ *     return; results are valid once `stream` reaches the point after the call.  With device-resident volumes and
  *     device outputs there is no host synchronisation inside.  Library-internal copy streams
  *     are joined to `stream` by events.
- *   - One host thread per handle at a time.  Different handles may be used concurrently.
+ *   - One host thread and one stream per handle at a time (the handle's device table, scratch and
+ *     staging buffers are single instances; order calls on different streams yourself).  Different
+ *     handles may be used concurrently.
  *   - There is no CPU fallback: without a CUDA device every compute call fails with VR_ERR_CUDA.
  */
 #ifndef VR_H_
