@@ -75,3 +75,39 @@ def test_random_cameras_and_options(be, seed):
                 assert np.array_equal(render(be, vol, sl, vr.VR_EA), ob.image, equal_nan=True), ("sort-last EA",) + tag
                 obm = O.render(v, sl, O.MIP, brick=B)
                 assert np.array_equal(render(be, vol, sl, vr.VR_MIP), obm.image), ("sort-last MIP",) + tag
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_random_summaries_and_statistics(be, seed):
+    """Random sizes, bin counts, caller ranges, layouts (linear, brick-major with halo on the device, out of core with a
+    random pool size and stream count), planted non-finite voxels: counts, min / max and the median bit-exact, the
+    float64 moments within 1e-13 of the data scale."""
+    from backends import statistics, summary
+    from test_parity import assert_statistics_equal, assert_summary_equal
+    rng = np.random.default_rng(2000 + seed)
+    for k in range(5):
+        n = tuple(int(x) for x in rng.integers(2, 48, size=3))
+        v = W.make_cube(W.Recipe(*n, seed=700 + seed * 8 + k, n_sources=int(rng.integers(0, 3)))).copy()
+        for _ in range(int(rng.integers(0, 4))):
+            v.reshape(-1)[int(rng.integers(0, v.size))] = rng.choice([np.nan, np.inf, -np.inf])
+        nbins = int(rng.choice([1, 7, 256, 1000, 4096]))
+        rng_arg = None if rng.random() < 0.5 else tuple(sorted(float(x) for x in rng.normal(size=2) * 2))
+        layout = int(rng.integers(0, 3))
+        B = int(rng.choice([4, 9, 16]))
+        kw = {}
+        if layout == 0:
+            data, lay = be.dev(v), vr.VR_LINEAR
+        else:
+            t = W.retile_halo(v, B)
+            lay = vr.VR_BRICKED_HALO1
+            if layout == 1:
+                data = be.dev(t)
+            else:
+                data = be.pinned(t)
+                n_bricks = int(np.prod([(d + B - 1) // B for d in n]))
+                if n_bricks > 2:
+                    kw = dict(resident_bytes=int(rng.integers(2, n_bricks)) * (B + 1) ** 3 * 4, n_copy_streams=int(rng.integers(1, 5)))
+        with vr.Volume(data, n, brick=B if layout else 0, layout=lay, **kw) as vol:
+            o = O.minmax_hist(v, nbins, rng_arg)
+            assert_summary_equal(summary(be, vol, nbins, rng_arg), o)
+            assert_statistics_equal(statistics(be, vol), O.statistics(v), v)
