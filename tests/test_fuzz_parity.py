@@ -111,3 +111,39 @@ def test_random_summaries_and_statistics(be, seed):
             o = O.minmax_hist(v, nbins, rng_arg)
             assert_summary_equal(summary(be, vol, nbins, rng_arg), o)
             assert_statistics_equal(statistics(be, vol), O.statistics(v), v)
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_random_chain_renders(be, seed):
+    """Brick-major volumes (resident and out of core, random brick edge, pool size and stream count) rendered brick by
+    brick with the ray state carried in the image, with and without the brick ranges of a prior summary pass (empty
+    bricks dropped), random pure perspective / orthographic cameras: bit-identical to the oracle's single march."""
+    from backends import summary
+    rng = np.random.default_rng(3000 + seed)
+    for k in range(4):
+        n, cam = _random_case(rng, 4 * (seed * 4 + k) + int(rng.integers(0, 3)))     # kinds 0, 1, 2: never mixed
+        if not (cam.is_perspective or cam.is_orthographic):
+            continue
+        B = int(rng.choice([3, 8, 16]))
+        v = W.make_cube(W.Recipe(*n, seed=900 + seed * 4 + k, n_sources=int(rng.integers(0, 3))))
+        s = O.minmax_hist(v)
+        tf = [W.tf_opaque(n, cam.step), W.tf_sources(n, cam.step, alpha_scale=10.0)][int(rng.integers(0, 2))]
+        t = W.retile_halo(v, B)
+        n_bricks = int(np.prod([(d + B - 1) // B for d in n]))
+        kw = {}
+        if rng.random() < 0.6 and n_bricks > 2:
+            data = be.pinned(t)
+            kw = dict(resident_bytes=int(rng.integers(2, n_bricks)) * (B + 1) ** 3 * 4, n_copy_streams=int(rng.integers(1, 5)))
+        else:
+            data = be.dev(t)
+        ert = float(rng.choice([0.0, 0.99]))
+        with vr.Volume(data, n, brick=B, layout=vr.VR_BRICKED_HALO1, **kw) as vol:
+            vol.set_transfer_function(tf, s.vmin, s.vmax)
+            if rng.random() < 0.6:
+                summary(be, vol)                                     # gathers the brick ranges: empty bricks get dropped
+            c2 = cam.with_(ert_alpha=ert)
+            oe = O.render(v, c2, O.EA, tf, s.vmin, s.vmax)
+            assert np.array_equal(render(be, vol, c2, vr.VR_EA), oe.image, equal_nan=True), (seed, k, n, B, kw, ert)
+            assert vol.stats()["path"] == 3
+            om = O.render(v, cam, O.MIP)
+            assert np.array_equal(render(be, vol, cam, vr.VR_MIP), om.image), (seed, k, n, B, kw)
