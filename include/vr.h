@@ -59,6 +59,10 @@ enum { VR_EA = 0,              /* emission-absorption, premultiplied RGBA, 4 cha
        VR_MIP = 1 };           /* maximum intensity projection, 1 channel */
 enum { VR_SORT_LAST = 1u };    /* vr_camera.flags: render per-brick partial images and merge them
                                   with the sort-last compositor even when a single march would do */
+/* vr_camera.flags: progressive pass — render only the pixels (i,j) with i % stride == phase_x and j % stride ==
+   phase_y, IN PLACE in the full-resolution image; stride 1..255, phases below the stride (see vr_render) */
+#define VR_SUBSAMPLE(stride, phase_x, phase_y) \
+    (((uint32_t)(stride) << 8) | ((uint32_t)(phase_x) << 16) | ((uint32_t)(phase_y) << 24))
 
 typedef struct vr_volume vr_volume; /* opaque; created and destroyed only by the library */
 
@@ -140,6 +144,13 @@ VR_API vr_status vr_set_transfer_function(vr_volume *vol, const float *rgba, flo
  *   flags      VR_SORT_LAST: per-brick partial images + compositor.  Needs brick > 0, a pure
  *              perspective or pure orthographic camera, and ert_alpha == 0 (early termination
  *              is not defined for independent partials, reading S15) => else VR_ERR_UNSUPPORTED.
+ *              VR_SUBSAMPLE(s, px, py): a progressive pass (the "interactive" of
+ *              PAPER.md:L34): only the pixels with i % s == px and j % s == py are rendered, into their own
+ *              places of the full-resolution image; every other pixel of the buffer is left untouched.  A rendered
+ *              pixel is bit-identical to the same pixel of a full render (the ray of pixel (i,j) is C.1's, whatever
+ *              the pass), so a viewer can show the s = 4 lattice while the camera moves (1/16 of the rays) and fill
+ *              in the remaining phases when it rests: after all s^2 phases the image IS the full render.  Single
+ *              march of a resident VR_LINEAR volume into a DEVICE image only (else VR_ERR_UNSUPPORTED).
  * Image: `pixels` is caller-owned, DEVICE (location VR_DEVICE) or pinned HOST (VR_HOST_PINNED;
  *   the library renders into an internal device image and enqueues the device-to-host copy on
  *   `stream`).  Row j = 0 is the v-minimum row; row_pitch_bytes >= width*channels*4 and a

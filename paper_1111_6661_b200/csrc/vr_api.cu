@@ -311,6 +311,7 @@ static CamK to_camk(const vr_camera *c)
     k.step = c->step;
     k.t_min = 1.0f - c->ert_alpha;        // one float32 subtraction (C.5)
     k.width = (int)c->width; k.height = (int)c->height;
+    k.sub = 1; k.sx = k.sy = 0;
     return k;
 }
 
@@ -852,6 +853,9 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     VR_REQUIRE(((uintptr_t)im->pixels & (mode == VR_EA ? 15u : 3u)) == 0, "image.pixels is misaligned");
     if (mode == VR_EA && !v->tf_set) { set_error("emission-absorption render before vr_set_transfer_function"); return VR_ERR_NOT_READY; }
     const bool sort_last = (c->flags & VR_SORT_LAST) != 0;
+    // progressive pass: only the pixels of one sub-lattice of the image, in place (VR_SUBSAMPLE)
+    const int sub = std::max(1, (int)((c->flags >> 8) & 0xffu)), sub_x = (int)((c->flags >> 16) & 0xffu), sub_y = (int)((c->flags >> 24) & 0xffu);
+    VR_REQUIRE(sub_x < sub && sub_y < sub, "VR_SUBSAMPLE: phase (%d, %d) must be below the stride %d", sub_x, sub_y, sub);
     const bool ert = mode == VR_EA && c->ert_alpha > 0.0f;
     const bool persp = zero3(c->ou) && zero3(c->ov), ortho = zero3(c->du) && zero3(c->dv);
     if (sort_last) {
@@ -860,6 +864,8 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
         if (v->out_of_core) { set_error("VR_SORT_LAST is not available for out-of-core volumes (they render as a chain)"); return VR_ERR_UNSUPPORTED; }
     }
     const bool need_plan = sort_last || v->out_of_core || v->desc.layout == VR_BRICKED_HALO1;
+    if (sub > 1 && need_plan) { set_error("VR_SUBSAMPLE is available for single-march renders of resident VR_LINEAR volumes only"); return VR_ERR_UNSUPPORTED; }
+    if (sub > 1 && im->location != VR_DEVICE) { set_error("VR_SUBSAMPLE renders in place: the image must be in device memory"); return VR_ERR_UNSUPPORTED; }
     if (need_plan && !persp && !ortho) { set_error("bricked rendering needs a pure perspective or pure orthographic camera"); return VR_ERR_UNSUPPORTED; }
 
     VR_CUDA(cudaSetDevice(v->device));
@@ -878,12 +884,23 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     if (rc != VR_OK) return rc;
 
     if (mode == VR_EA) { rc = upload_tf(v, st); if (rc != VR_OK) return rc; }
-    const CamK cam = to_camk(c);
+    CamK cam = to_camk(c);
+    vr_camera lattice = *c;                  // the camera of the pixels this call renders (lane map, class probes)
+    if (sub > 1) {
+        cam.sub = sub; cam.sx = sub_x; cam.sy = sub_y;
+        cam.width = ((int)c->width - sub_x + sub - 1) / sub; cam.height = ((int)c->height - sub_y + sub - 1) / sub;
+        lattice.width = (uint32_t)std::max(cam.width, 0); lattice.height = (uint32_t)std::max(cam.height, 0);
+        for (int a = 0; a < 3; ++a) {
+            lattice.o0[a] += (float)sub_x * c->ou[a] + (float)sub_y * c->ov[a]; lattice.d0[a] += (float)sub_x * c->du[a] + (float)sub_y * c->dv[a];
+            lattice.ou[a] *= (float)sub; lattice.ov[a] *= (float)sub; lattice.du[a] *= (float)sub; lattice.dv[a] *= (float)sub;
+        }
+        if (cam.width <= 0 || cam.height <= 0) return VR_OK;        // the sub-lattice has no pixel in this image
+    }
     TfK tf; tf.table = v->d_tf; tf.scale = v->tf_scale; tf.bias = v->tf_bias;
     if (sort_last) rc = render_sort_last(v, c, cam, mode, tf, img, pitch_f, st);
     else if (v->out_of_core || v->desc.layout == VR_BRICKED_HALO1) rc = render_chain(v, c, cam, mode, ert, tf, img, pitch_f, st);
     else if (v->opt_path == 1 || !lanes_addressable(v)) rc = render_single(v, cam, mode, ert, tf, img, pitch_f, st);
-    else rc = render_lanes(v, c, cam, mode, ert, tf, nullptr, img, pitch_f, st);
+    else rc = render_lanes(v, &lattice, cam, mode, ert, tf, nullptr, img, pitch_f, st);
     if (rc != VR_OK) return rc;
     VR_CUDA(cudaGetLastError());
     if (im->location == VR_HOST_PINNED) {

@@ -182,8 +182,9 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__re
     // pixel of this lane: p along the lane axis, q = sheared row + off(p)
     const int p = blockIdx.x * 32 + lane;
     const int q = M.q_lo + (int)blockIdx.y * kRowsPerCta + warp + __float2int_rd(__fmaf_rn(M.sigma, (float)p, 0.5f));
-    const int i = M.lane_axis == 0 ? p : q, j = M.lane_axis == 0 ? q : p;
-    const bool inside = i >= 0 && i < cam.width && j >= 0 && j < cam.height;
+    const int li = M.lane_axis == 0 ? p : q, lj = M.lane_axis == 0 ? q : p;      // pixel of the (sub-)lattice
+    const bool inside = li >= 0 && li < cam.width && lj >= 0 && lj < cam.height;
+    const int i = li * cam.sub + cam.sx, j = lj * cam.sub + cam.sy;              // image pixel (C.1 uses these)
     Ray r;
     bool mine = false, alive = false;
     if (inside) {

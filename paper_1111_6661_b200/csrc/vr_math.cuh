@@ -45,7 +45,8 @@ struct CamK {                       // kernel-side copy of vr_camera (C.1)
     float o0[3], ou[3], ov[3], d0[3], du[3], dv[3];
     float step;
     float t_min;                    // 1 - ert_alpha, rounded once (C.5)
-    int width, height;
+    int width, height;              // the pixels this render produces: the whole image, or the lattice of a progressive pass
+    int sub, sx, sy;                // progressive pass (VR_SUBSAMPLE): lattice pixel (i', j') is image pixel (sub i' + sx, sub j' + sy)
 };
 
 struct VolK {                       // the voxel box and how to address it

@@ -87,6 +87,7 @@ k_march_full(CamK cam, VolK V, TfK tf, float *__restrict__ image, long long pitc
     int i, j;
     thread_pixel(blockIdx.x, blockIdx.y, i, j);
     if (i >= cam.width || j >= cam.height) return;
+    i = i * cam.sub + cam.sx; j = j * cam.sub + cam.sy;          // progressive pass: lattice pixel -> image pixel
     Ray r;
     Accum A = { 0.0f, 0.0f, 0.0f, 1.0f, -CUDART_INF_F };
     if (make_ray(cam, V.nx, V.ny, V.nz, i, j, r)) march<MODE, ERT, WIDE, false>(V, r, cam, tf_s, tf.scale, tf.bias, 0, -1, A);

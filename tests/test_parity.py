@@ -485,6 +485,56 @@ def test_16_byte_row_loads(be, n, wide):
         assert vol.stats()["path"] == 7
 
 
+@pytest.mark.parametrize("path", [0, 1])
+def test_progressive_passes(be, path):
+    """VR_SUBSAMPLE: a pass renders one sub-lattice of the pixels in place; every rendered pixel is bit-identical to the
+    oracle's pixel (its `mask` is the same lattice), every other pixel of the buffer is untouched, and after all
+    stride^2 phases the buffer IS the full render.  Views with both pixel classes, an image that is not a multiple of
+    the stride, a phase without any pixel."""
+    n = (52, 40, 61)
+    v = W.make_cube(W.Recipe(*n, seed=71, n_sources=4))
+    s = O.minmax_hist(v)
+    tf = W.tf_opaque(n, 0.5)
+    cams = [c.with_(ert_alpha=0.99) for k, c in _axis_views(n, False) if k in ("persp0", "persp6", "ortho_z")]
+    with vr.Volume(be.dev(v), n) as vol:
+        vol.set_option(vr.VR_OPT_RENDER_PATH, path)
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        for cam in cams:
+            H, Wd = cam.height, cam.width
+            full = O.render(v, cam, O.EA, tf, s.vmin, s.vmax).image
+            for stride in (4, 3):
+                buf = be.empty((H, Wd, 4), fill=7.0)
+                seen = np.zeros((H, Wd), dtype=bool)
+                for py in range(stride):
+                    for px in range(stride):
+                        vol.render(cam.with_(flags=vr.VR_SUBSAMPLE(stride, px, py)), vr.VR_EA, out=buf, stream=be.stream)
+                        seen[py::stride, px::stride] = True
+                        g = be.numpy(buf)
+                        assert np.array_equal(g[seen], full[seen]) and (g[~seen] == 7.0).all(), (stride, px, py)
+                        if (px, py) == (0, 0):                   # the oracle with the same lattice as its mask
+                            mask = seen.astype(np.uint8)
+                            o = O.render(v, cam, O.EA, tf, s.vmin, s.vmax, mask=mask).image
+                            assert np.array_equal(g[seen], o[seen])
+                assert np.array_equal(be.numpy(buf), full)
+            mbuf = be.empty((H, Wd), fill=-3.0)
+            vol.render(cam.with_(flags=vr.VR_SUBSAMPLE(5, 2, 1)), vr.VR_MIP, out=mbuf, stream=be.stream)
+            gm, om = be.numpy(mbuf), O.render(v, cam, O.MIP).image
+            assert np.array_equal(gm[1::5, 2::5], om[1::5, 2::5]) and (np.delete(np.delete(gm, np.s_[1::5], 0), np.s_[2::5], 1) == -3.0).all()
+        tiny = cams[0].with_(width=3, height=2)
+        tb = be.empty((2, 3, 4), fill=7.0)
+        vol.render(tiny.with_(flags=vr.VR_SUBSAMPLE(4, 3, 3)), vr.VR_EA, out=tb, stream=be.stream)     # no pixel has j % 4 == 3
+        assert (be.numpy(tb) == 7.0).all()
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cams[0].with_(flags=vr.VR_SUBSAMPLE(2, 2, 0)), vr.VR_EA, out=tb, stream=be.stream)
+        assert e.value.status == vr.VR_ERR_INVALID_ARG
+    with vr.Volume(be.dev(v), n, brick=16) as vol:
+        vol.set_transfer_function(tf, s.vmin, s.vmax)
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cams[0].with_(ert_alpha=0.0, flags=vr.VR_SUBSAMPLE(2, 0, 0) | vr.VR_SORT_LAST), vr.VR_EA,
+                       out=be.empty((cams[0].height, cams[0].width, 4)), stream=be.stream)
+        assert e.value.status == vr.VR_ERR_UNSUPPORTED
+
+
 def test_mixed_camera_renders(be):
     """A camera whose origins AND directions vary per pixel (neither perspective nor orthographic)."""
     n = (32, 32, 32)
