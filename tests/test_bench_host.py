@@ -158,6 +158,7 @@ def test_bench_flow_and_json_line_in_emulation(number, scale, capsys):
     c = printed["cpu_baseline"]
     assert c["kind"] == "oracle" and c["value"] > 0 and c["cores"] >= 1 and "sample" in c
     if number != 5:
+        assert printed["data_passes"]["summary_ms"] > 0 and printed["data_passes"]["statistics_gbs"] > 0
         assert printed["render_ms_cold"] is not None or cfg.sort_last
         assert len(printed["render_ms_by_view"]) == 2 * len(cfg.modes)
 
