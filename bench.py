@@ -354,8 +354,8 @@ def run_ours(args, rig=None, cfg=None):
         vol.set_option(vr.VR_OPT_LANE_LAG, args.lag)
     if args.no_zcopy:
         vol.set_option(vr.VR_OPT_ZFAST_COPY, 0)
-    if args.quad:
-        vol.set_option(vr.VR_OPT_ROW_LOADS, 1)
+    if args.row_loads >= 0:
+        vol.set_option(vr.VR_OPT_ROW_LOADS, args.row_loads)
     sbuf = rig.dev_empty((32 + 8 * 256,), np.uint8)
     vol.minmax_histogram(256, out=sbuf, stream=rig.stream_arg)
     s = read_summary(rig, sbuf)
@@ -729,7 +729,7 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="VR_OPT_RENDER_PATH for ablations (0 = auto, the product default)")
     ap.add_argument("--lag", type=int, default=-1, help="VR_OPT_LANE_LAG for ablations (-1 = library default)")
     ap.add_argument("--no-zcopy", action="store_true", help="VR_OPT_ZFAST_COPY = 0 (ablation)")
-    ap.add_argument("--quad", action="store_true", help="VR_OPT_ROW_LOADS = 1: one 16-byte load per row (ablation; see profiles/r2_lane_traffic_model.md)")
+    ap.add_argument("--row-loads", type=int, default=-1, help="VR_OPT_ROW_LOADS for ablations: 0 scalar, 1 16-byte quads, 2 auto (-1 = library default, auto)")
     ap.add_argument("--views", type=int, default=0, help="render only the first N views of the orbit (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":

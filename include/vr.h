@@ -321,10 +321,13 @@ VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
  *                       C.5), so images are bit-identical.  Used only while at least 1/64 of the cells are
  *                       empty (decided on the device, no read-back).  0: never.
  *   VR_OPT_ROW_LOADS    lane-mapped path: how the two voxels (u, u+1) a sample reads from each of its four rows are
- *                       fetched.  0 (default): two 4-byte loads.  1: ONE aligned 16-byte load of the quad that holds u,
- *                       plus a 4-byte load of u+1 for the lanes whose u ends its quad — fewer cache lines touched per
- *                       sample on oblique views, more select instructions (profiles/r2_lane_traffic_model.md); used when
- *                       the memory-fast dimension is a multiple of 4, ignored with empty-space skipping and sort-last.
+ *                       fetched.  0: two 4-byte loads.  1: ONE aligned 16-byte load of the quad that holds u, plus a
+ *                       4-byte load of u+1 for the lanes whose u ends its quad — fewer cache lines touched per sample,
+ *                       more select instructions.  2 (default): 1 for the launches whose rays can enter the volume
+ *                       through a face perpendicular to the memory-fast axis (oblique views: bound by lines touched),
+ *                       0 for the others (bound by instruction issue); see profiles/r2_lane_traffic_model.md.  Quads
+ *                       need a memory-fast dimension that is a multiple of 4 and are not used with empty-space
+ *                       skipping or sort-last.
  *   VR_OPT_FORCE_WIDE   1: the render kernels form 64-bit voxel offsets even for volumes of fewer than 2^32
  *                       voxels (the code the largest volumes run; lets the tests cover it at small size).  Default 0.
  * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).

@@ -124,7 +124,7 @@ struct vr_volume {
     float *zfast = nullptr;
     bool zfast_failed = false;                // allocation refused once: not retried
     cudaEvent_t zfast_ev = nullptr;           // recorded after the transposition
-    int opt_path = 0, opt_zcopy = 1, opt_lag = 1, opt_wide = 0, opt_quad = 0;   // vr_set_option
+    int opt_path = 0, opt_zcopy = 1, opt_lag = 1, opt_wide = 0, opt_quad = 2;   // vr_set_option
     Staging staging[kStagingRing];
     int staging_next = 0;
 
@@ -616,6 +616,21 @@ static bool lanes_addressable(const vr_volume *v)
     return (uint64_t)v->desc.nx * v->desc.ny <= 0xffffffffull && (uint64_t)v->desc.ny * v->desc.nz <= 0xffffffffull;
 }
 
+// VR_OPT_ROW_LOADS = 2 (auto): 16-byte row loads for the launches whose rays can enter the volume through a face
+// perpendicular to the memory-fast axis of the copy they read.  Those are the oblique views, where the lanes of a
+// warp sit on rows of their own and the corner loads are bound by cache lines touched (3.5-4.6 lines per sample
+// with two scalar loads per row, 2.6-3.1 with one quad: profiles/r2_lane_traffic_model.md); on the other views the
+// lanes share rows, issue binds, and the selects of the quad variant cost more than its lines save.  A face is
+// visible iff the eye is beyond it (perspective) or the direction has a component along its axis (orthographic).
+static bool launch_quad(const vr_volume *v, const vr_camera *c, int fast)
+{
+    if (v->opt_quad != 2) return v->opt_quad == 1;
+    const float n_fast = (float)(fast == 0 ? v->desc.nx : v->desc.nz);
+    if (zero3(c->ou) && zero3(c->ov)) return c->o0[fast] < 0.0f || c->o0[fast] > n_fast;
+    if (zero3(c->du) && zero3(c->dv)) return c->d0[fast] != 0.0f;
+    return true;
+}
+
 // part != nullptr: per-(ray, owner brick) fragments for the sort-last compositor instead of pixels
 static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam, int mode, bool ert, const TfK &tf,
                               const PartK *part, float *img, long long pitch_f, cudaStream_t st)
@@ -643,17 +658,17 @@ static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam,
     int rows;
     if (!have_z || n_x == 0) {
         make_lane_map(c, n, 0, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, v->opt_quad != 0, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 0), rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else if (n_x == 9) {
         make_lane_map(c, n, 2, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, v->opt_quad != 0, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 2), rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else {
         make_lane_map(c, n, 0, 1, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, v->opt_quad != 0, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 0), rows, img, pitch_f, st);
         make_lane_map(c, n, 2, 2, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, v->opt_quad != 0, rows, img, pitch_f, st);
+        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 2), rows, img, pitch_f, st);
         v->stats.kernel_launches += 2;
     }
     v->stats.path = 7;
@@ -1095,7 +1110,7 @@ VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
         VR_REQUIRE(value >= 0 && value <= 1024, "VR_OPT_LANE_LAG: 0..1024 base planes (got %lld)", (long long)value);
         v->opt_lag = (int)value; return VR_OK;
     case VR_OPT_ROW_LOADS:
-        VR_REQUIRE(value == 0 || value == 1, "VR_OPT_ROW_LOADS: 0 scalar, 1 one 16-byte load per row (got %lld)", (long long)value);
+        VR_REQUIRE(value >= 0 && value <= 2, "VR_OPT_ROW_LOADS: 0 scalar, 1 one 16-byte load per row, 2 auto (got %lld)", (long long)value);
         v->opt_quad = (int)value; return VR_OK;
     case VR_OPT_FORCE_WIDE:
         VR_REQUIRE(value == 0 || value == 1, "VR_OPT_FORCE_WIDE: 0 or 1 (got %lld)", (long long)value);

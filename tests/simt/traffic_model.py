@@ -38,6 +38,7 @@ def run(cfg, v, cam, mode, variant):
             vol.set_option(vr.VR_OPT_ZFAST_COPY, zcopy)
             vol.set_option(vr.VR_OPT_LANE_LAG, lag)
             vol.set_option(vr.VR_OPT_EMPTY_SKIP, 0)
+            vol.set_option(vr.VR_OPT_ROW_LOADS, 0)                   # the trace counts the scalar loads (+ the quad what-if)
             vol.set_transfer_function(W.tf_haze(cfg.dims, cfg.step), -6.0, 24.0)
             out = simt_lib.Buffer((cam.height, cam.width, 4) if mode == vr.VR_EA else (cam.height, cam.width))
             lib.simt_trace(1)

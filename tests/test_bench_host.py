@@ -125,7 +125,7 @@ class SimtRig:
 def _args(**kw):
     import argparse
     d = dict(gpus=1, steps=1, warmup=1, impl="ours", config=2, no_cpu=False, no_e2e=False, cpu_seconds=0.3, ooc_nz=0,
-             ooc_resident_frac=0.25, path=0, lag=-1, no_zcopy=False, quad=False, views=2)
+             ooc_resident_frac=0.25, path=0, lag=-1, no_zcopy=False, row_loads=-1, views=2)
     d.update(kw)
     return argparse.Namespace(**d)
 

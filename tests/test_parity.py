@@ -551,7 +551,7 @@ def test_set_option_rejects_bad_values(be):
     v = W.make_cube(W.Recipe(16, 16, 16, seed=1))
     with vr.Volume(be.dev(v), (16, 16, 16)) as vol:
         for opt, val in ((vr.VR_OPT_RENDER_PATH, 5), (vr.VR_OPT_ZFAST_COPY, 2), (vr.VR_OPT_LANE_LAG, -1),
-                         (vr.VR_OPT_EMPTY_SKIP, 2), (vr.VR_OPT_FORCE_WIDE, -1), (vr.VR_OPT_ROW_LOADS, 2), (77, 0)):
+                         (vr.VR_OPT_EMPTY_SKIP, 2), (vr.VR_OPT_FORCE_WIDE, -1), (vr.VR_OPT_ROW_LOADS, 3), (77, 0)):
             with pytest.raises(vr.VrError) as e:
                 vol.set_option(opt, val)
             assert e.value.status == vr.VR_ERR_INVALID_ARG
