@@ -326,8 +326,8 @@ VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
  *                       more select instructions.  2 (default): 1 for the launches whose rays can enter the volume
  *                       through a face perpendicular to the memory-fast axis (oblique views: bound by lines touched),
  *                       0 for the others (bound by instruction issue); see profiles/r2_lane_traffic_model.md.  Quads
- *                       need a memory-fast dimension that is a multiple of 4 and are not used with empty-space
- *                       skipping or sort-last.
+ *                       need a memory-fast dimension that is a multiple of 4 and are not used by the empty-space
+ *                       skipping variant.
  *   VR_OPT_FORCE_WIDE   1: the render kernels form 64-bit voxel offsets even for volumes of fewer than 2^32
  *                       voxels (the code the largest volumes run; lets the tests cover it at small size).  Default 0.
  * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).

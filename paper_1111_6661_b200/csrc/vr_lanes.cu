@@ -308,14 +308,15 @@ void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int f
     const bool wide = force_wide || span > 0xffffffffull;
     const bool skip = mode == VR_EA && macro.flag != nullptr && !part;
     // 16-byte row loads need rows that start 16-byte aligned (the base is, vr_create_volume) and hold a multiple of 4
-    const bool quad = quad_loads && !skip && !part && ((fast == 0 ? vol.nx : vol.nz) & 3) == 0 &&
+    const bool quad = quad_loads && !skip && ((fast == 0 ? vol.nx : vol.nz) & 3) == 0 &&
                       (((uintptr_t)vol.base) & 15u) == 0;
     PartK P;
     if (part) P = *part;
     else { P.bricks = nullptr; P.lut = nullptr; P.arena = nullptr; P.B = 1; P.nbx = P.nby = 0; }
 #define VR_L4(M, E, Wd, F, S) vr_launch(k_rows<M, E, Wd, F, S, false, false>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f)
 #define VR_L3(M, E, Wd, F) do { \
-        if (part) vr_launch(k_rows<M, false, Wd, F, false, true, false>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f); \
+        if (part && quad) vr_launch(k_rows<M, false, Wd, F, false, true, true>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f); \
+        else if (part) vr_launch(k_rows<M, false, Wd, F, false, true, false>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f); \
         else if (quad) vr_launch(k_rows<M, E, Wd, F, false, false, true>, g, kLaneThreads, 0, st, cam, vol, tf, map, macro, P, image, pitch_f); \
         else if (M == VR_EA && skip) VR_L4(M, E, Wd, F, (M == VR_EA)); else VR_L4(M, E, Wd, F, false); } while (0)
 #define VR_L2(M, E, Wd) do { if (fast == 0) VR_L3(M, E, Wd, 0); else VR_L3(M, E, Wd, 2); } while (0)

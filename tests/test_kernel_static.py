@@ -65,9 +65,10 @@ def test_ray_caster_resources(sass, resources):
     transfer function is the only shared memory; 8 corner loads per sample (+ 1 byte of the skipping grid); packed
     FFMA2 lerps."""
     rows = {k: v for k, v in resources.items() if "k_rows<" in k}
-    assert len(rows) == 40                                            # MIP 4 + EA 8 + EA skip 8 + partials 8 + 16-byte loads 12
+    assert len(rows) == 48                                            # MIP 4 + EA 8 + EA skip 8 + partials 8 + 16-byte loads 12 + 8 (partials)
     for k, (reg, stack, shared, local) in rows.items():
-        assert reg <= 48 and shared <= 5200, (k, reg, shared)
+        partials_with_quads = k.split(">(")[0].endswith("true, true")          # the one variant above 48: 4 CTAs per SM
+        assert reg <= (64 if partials_with_quads else 48) and shared <= 5200, (k, reg, shared)
     for k, ops in sass.items():
         if "k_rows<" not in k:
             continue
@@ -77,7 +78,7 @@ def test_ray_caster_resources(sass, resources):
         mode, ert, wide, fast, skip, part, quad = (int(x) if x.isdigit() else x == "true" for x in args.groups())
         n_corner = len([op for op in ldg if ".U8" not in op and ".128" not in op and ".64" not in op])
         if part:                                                      # + the brick table reads of the two fragment flushes
-            assert 8 <= n_corner <= 24, (k, ldg)
+            assert (4 if quad else 8) <= n_corner <= 24, (k, ldg)
         elif quad:                                                    # 4 quads + 4 predicated scalars (+ the staged table)
             assert n_corner == 4 and len([op for op in ldg if ".128" in op]) >= 4, (k, ldg)
         else:

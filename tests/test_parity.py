@@ -568,12 +568,12 @@ def test_all_miss_camera(be):
 
 
 # ------------------------------------------------------------------ bricks: A0, A4, A10
-@pytest.mark.parametrize("B,how", [(7, "lanes"), (16, "lanes"), (32, "lanes"), (100, "lanes"), (16, "tiles"), (16, "halo")])
+@pytest.mark.parametrize("B,how", [(7, "lanes"), (16, "lanes"), (32, "lanes"), (100, "lanes"), (16, "quads"), (16, "tiles"), (16, "halo")])
 def test_sort_last_equals_oracle_bricked(be, B, how):
     """Fragments from the lane-mapped march that flushes at every change of owner brick (`lanes`, the default for
     linear volumes), from one CTA per (brick, pixel tile) on a linear volume (`tiles`) and on a resident brick-major
     volume with halo (`halo`): all bit-identical to the oracle's bricked render (same partials, same fold order)."""
-    n = (61, 47, 83)
+    n = (60, 47, 84) if how == "quads" else (61, 47, 83)            # quads need nx and nz to be multiples of 4
     v = W.make_cube(W.Recipe(*n, seed=33, n_sources=5))
     s = O.minmax_hist(v)
     R = float(max(abs(s.vmin), abs(s.vmax)))
@@ -582,6 +582,8 @@ def test_sort_last_equals_oracle_bricked(be, B, how):
     with vr.Volume(data, n, brick=B, layout=vr.VR_BRICKED_HALO1 if how == "halo" else vr.VR_LINEAR) as vol:
         if how == "tiles":
             vol.set_option(vr.VR_OPT_RENDER_PATH, vr.VR_PATH_RAY_MAJOR)
+        if how == "quads":
+            vol.set_option(vr.VR_OPT_ROW_LOADS, 1)
         vol.set_transfer_function(tf, s.vmin, s.vmax)
         for name, cam in _views(n):
             cam = cam.with_(flags=W.cameras.VR_SORT_LAST)
