@@ -66,7 +66,7 @@ def main():
           "spacing in voxels — what decides coalescing — is the config's own).\n")
     print("`lines / sample` = 8 loads x lines per load / active lanes: the L1 cost of one sample.  `what-if 16 B` = the same with "
           "ONE aligned 16-byte load per row (+ a scalar load for the lanes whose x is the last element of its quad) instead of "
-          "two scalar loads: a variant that is not built (DESIGN.md §10), counted here to size its gain.\n")
+          "two scalar loads: what `k_rows<QUAD>` (VR_OPT_ROW_LOADS) does, counted from the scalar trace.\n")
     print("| config (scale) | view | variant | samples | lane efficiency | lines / load | sectors / load | lines / sample | what-if 16 B: lines / sample |")
     print("|---|---|---|---:|---:|---:|---:|---:|---:|")
     for number in (int(x) for x in args.configs.split(",")):
