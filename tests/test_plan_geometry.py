@@ -10,8 +10,12 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def test_brick_rectangles_and_visibility_order(tmp_path):
     exe = str(tmp_path / "plan_check")
-    subprocess.run(["g++", "-O2", "-std=c++17", "-o", exe, os.path.join(ROOT, "tests", "plan_check.cpp")], check=True,
+    subprocess.run(["g++", "-O2", "-std=c++17", "-mfma", "-ffp-contract=off", "-o", exe, os.path.join(ROOT, "tests", "plan_check.cpp")], check=True,
                    capture_output=True)
     r = subprocess.run([exe, "80"], capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "rect_bad 0" in r.stdout and "order_bad 0" in r.stdout
+    # the same at the sizes, brick edges, images and orbit cameras of cfg3 / cfg4 / cfg5, with float32 rays (C.1-C.3)
+    r = subprocess.run([exe, "0", "configs"], capture_output=True, text=True)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "rect_bad 0" in r.stdout and "order_bad 0" in r.stdout
