@@ -2,6 +2,7 @@
 // formula of k_rows in csrc/vr_lanes.cu): for random perspective, orthographic and mixed cameras and image
 // sizes, every pixel of the image is produced by exactly one (CTA, warp, lane) of the launched grid, for
 // both volume copies and every pixel class.  Also reports how well the shear follows the fast axis.
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <random>
@@ -56,6 +57,49 @@ int main(int argc, char **argv)
                 ++cams;
             }
     }
+    // the configs' own images and orbit cameras (workload/cameras.py): 1024^2, 1920x1080, 3840x2160, 8 views each
+    const int sizes[3][5] = { { 1024, 1024, 512, 512, 1024 }, { 1920, 1080, 1024, 1024, 2048 }, { 3840, 2160, 2048, 2048, 4096 } };
+    for (int si = 0; si < 3; ++si)
+        for (int view = 0; view < 8; ++view) {
+            const int W = sizes[si][0], H = sizes[si][1], n[3] = { sizes[si][2], sizes[si][3], sizes[si][4] };
+            const double c[3] = { n[0] / 2.0, n[1] / 2.0, n[2] / 2.0 };
+            const double rb = 0.5 * std::sqrt((double)n[0] * n[0] + (double)n[1] * n[1] + (double)n[2] * n[2]);
+            const double R = rb / std::sin(M_PI / 8.0), th = 2.0 * M_PI * (view + 0.25) / 8.0, el = M_PI / 9.0;
+            const double eye[3] = { c[0] + R * std::cos(el) * std::sin(th), c[1] + R * std::sin(el), c[2] + R * std::cos(el) * std::cos(th) };
+            double f[3] = { c[0] - eye[0], c[1] - eye[1], c[2] - eye[2] };
+            const double fl = std::sqrt(f[0] * f[0] + f[1] * f[1] + f[2] * f[2]);
+            for (double &x : f) x /= fl;
+            double r[3] = { f[1] * 0 - f[2] * 1, f[2] * 0 - f[0] * 0, f[0] * 1 - f[1] * 0 };      // f x (0,1,0)
+            const double rl = std::sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
+            for (double &x : r) x /= rl;
+            const double u[3] = { r[1] * f[2] - r[2] * f[1], r[2] * f[0] - r[0] * f[2], r[0] * f[1] - r[1] * f[0] };
+            const double tf = std::tan(M_PI / 8.0), asp = (double)W / H;
+            vr_camera cam{};
+            cam.struct_size = sizeof(cam); cam.width = (unsigned)W; cam.height = (unsigned)H; cam.step = 1.0f;
+            for (int a = 0; a < 3; ++a) {
+                cam.o0[a] = (float)eye[a];
+                cam.d0[a] = (float)(f[a] - tf * asp * r[a] - tf * u[a]);
+                cam.du[a] = (float)(2.0 * tf * asp / W * r[a]); cam.dv[a] = (float)(2.0 * tf / H * u[a]);
+            }
+            for (int fast = 0; fast <= 2; fast += 2) {
+                LaneMapK M;
+                int rows;
+                make_lane_map(&cam, n, fast, fast == 0 ? 1 : 2, 1, M, rows);
+                const int P = M.lane_axis == 0 ? W : H;
+                std::vector<unsigned char> cnt((size_t)W * H, 0);
+                const int gx = (P + 31) / 32, gy = (rows + 7) / 8;
+                for (int by = 0; by < gy; ++by)
+                    for (int bx = 0; bx < gx; ++bx)
+                        for (int t = 0; t < 256; ++t) {
+                            const int p = bx * 32 + (t & 31);
+                            const int q = M.q_lo + by * 8 + (t >> 5) + lane_row_offset(M.sigma, p);
+                            const int i = M.lane_axis == 0 ? p : q, j = M.lane_axis == 0 ? q : p;
+                            if (i >= 0 && i < W && j >= 0 && j < H) cnt[(size_t)j * W + i]++;
+                        }
+                for (unsigned char v : cnt) if (v != 1) ++bad;
+                ++cams;
+            }
+        }
     printf("maps %lld bad %lld\n", cams, bad);
     return bad ? 1 : 0;
 }
