@@ -53,7 +53,8 @@ inline void vr_launch(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, 
 #else
 #define VR_TRACE_CORNER_LOADS(active, base, p0, p1, p2, p3) ((void)0)
 #endif
-enum { VR_CNT_LEAP_CELL = 0, VR_CNT_LEAP_BLOCK = 1, VR_CNT_LEAP_REJECTED = 2, VR_CNT_LAG_WAIT = 3 };
+enum { VR_CNT_LEAP_CELL = 0, VR_CNT_LEAP_BLOCK = 1, VR_CNT_LEAP_REJECTED = 2, VR_CNT_LAG_WAIT = 3, VR_CNT_FRAG_OUTSIDE = 4,
+       VR_CNT_FRAG_NO_BRICK = 5 };
 
 // dynamic shared memory of the CTA as an array of T
 #ifdef VR_SIMT_HOST

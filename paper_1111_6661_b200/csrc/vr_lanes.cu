@@ -160,7 +160,7 @@ __device__ __forceinline__ void flush_fragment(const PartK &P, int cur, int i, i
 {
     const BrickK *b = P.bricks + cur;
     const int x0 = __ldg(&b->x0), y0 = __ldg(&b->y0), x1 = __ldg(&b->x1), y1 = __ldg(&b->y1);
-    if (i < x0 || i >= x1 || j < y0 || j >= y1) return;          // never: the screen rectangle holds every owning pixel (A4)
+    if (i < x0 || i >= x1 || j < y0 || j >= y1) { VR_TEST_COUNT(VR_CNT_FRAG_OUTSIDE); return; }   // never: the rectangle holds every owning pixel (A4)
     const unsigned long long f = __ldg(&b->frag_off) + (unsigned long long)(j - y0) * (unsigned)(x1 - x0) + (unsigned)(i - x0);
     if (MODE == VR_MIP) P.arena[f] = m;
     else reinterpret_cast<float4 *>(P.arena)[f] = make_float4(cr, cg, cb, T);
@@ -233,6 +233,7 @@ k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__re
             if (cur >= 0) flush_fragment<MODE>(P, cur, i, j, cr, cg, cb, T, m);
             const int bx = ix / P.B, by = iy / P.B, bz = iz / P.B;
             cur = __ldg(P.lut + (bz * P.nby + by) * P.nbx + bx);
+            if (cur < 0) VR_TEST_COUNT(VR_CNT_FRAG_NO_BRICK);      // never: a brick that owns a sample is in the plan (A4)
             blo[0] = bx * P.B; blo[1] = by * P.B; blo[2] = bz * P.B;
             bhi[0] = blo[0] + P.B - 1; bhi[1] = blo[1] + P.B - 1; bhi[2] = blo[2] + P.B - 1;
             cr = cg = cb = 0.0f; T = 1.0f; m = -CUDART_INF_F;

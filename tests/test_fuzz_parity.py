@@ -46,6 +46,9 @@ def _random_case(rng, k):
 @pytest.mark.parametrize("seed", range(6))
 def test_random_cameras_and_options(be, seed):
     rng = np.random.default_rng(1000 + seed)
+    if be.name == "simt":
+        import simt_lib
+        simt_lib.lib().simt_reset_counters()
     for k in range(8 if be.full else 5):
         n, cam = _random_case(rng, seed * 8 + k)
         v = W.make_cube(W.Recipe(*n, seed=500 + seed * 8 + k, n_sources=int(rng.integers(0, 4))))
@@ -75,6 +78,8 @@ def test_random_cameras_and_options(be, seed):
                 assert np.array_equal(render(be, vol, sl, vr.VR_EA), ob.image, equal_nan=True), ("sort-last EA",) + tag
                 obm = O.render(v, sl, O.MIP, brick=B)
                 assert np.array_equal(render(be, vol, sl, vr.VR_MIP), obm.image), ("sort-last MIP",) + tag
+    if be.name == "simt":                # sort-last: every fragment inside its rectangle, every owner brick in the plan
+        assert simt_lib.lib().simt_counter(4) == 0 and simt_lib.lib().simt_counter(5) == 0
 
 
 @pytest.mark.parametrize("seed", range(4))

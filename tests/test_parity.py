@@ -579,6 +579,9 @@ def test_sort_last_equals_oracle_bricked(be, B, how):
     R = float(max(abs(s.vmin), abs(s.vmax)))
     tf = W.bake_tf(W.TF_HAZE_POINTS, 0.5, alpha_scale=6.0)
     data = be.dev(W.retile_halo(v, B)) if how == "halo" else be.dev(v)
+    if be.name == "simt":
+        import simt_lib
+        simt_lib.lib().simt_reset_counters()
     with vr.Volume(data, n, brick=B, layout=vr.VR_BRICKED_HALO1 if how == "halo" else vr.VR_LINEAR) as vol:
         if how == "tiles":
             vol.set_option(vr.VR_OPT_RENDER_PATH, vr.VR_PATH_RAY_MAJOR)
@@ -596,6 +599,8 @@ def test_sort_last_equals_oracle_bricked(be, B, how):
             assert se["bit_exact"] == 1.0, (name, se)                # same partials, same fold order
             st = vol.stats()
             assert st["path"] == 2 and st["fragments"] > 0
+    if be.name == "simt":                # no fragment fell outside its brick's rectangle, no owner brick was missing from the plan
+        assert simt_lib.lib().simt_counter(4) == 0 and simt_lib.lib().simt_counter(5) == 0
 
 
 def test_sort_last_rejections(be):
