@@ -6,9 +6,11 @@
  * includes none of its headers.
  *
  * The paper names the operation — ray-cast volume rendering
- * of float spectral cubes, plus min/max and histogram — but
- * gives no formulae; every step below follows the readings fixed in SURVEY.md
- * §8(c) C.0–C.8 (listed again in DESIGN.md §3), in that order and notation.
+ * of float spectral cubes, plus min/max and histogram, median
+ * and standard deviation (L66), a viewer that only displays results (L48, L70) —
+ * but gives no formulae; every step below follows the readings fixed in SURVEY.md
+ * §8(c) C.0–C.8 and DESIGN.md §3 C.13 (statistics), C.14 (8-bit frame), S41
+ * (histogram ranges that overflow the bin arithmetic), in that order and notation.
  *
  * Two precisions:
  *   f32-canonical (the parity gate): the exact binary32 operation sequence of
@@ -21,7 +23,10 @@
  * unbricked; P4 min/max/hist == brute force; P5 affine cube; P6 impulse tent;
  * P7 alpha 0 / alpha 1; P8 sample counts; P9/P10 mirror symmetry; P11 ERT bound;
  * P12 f32 vs f64 distance; P13 step-halving convergence; P14 halo layout; P15
- * non-finite voxels in a render (S24).  No function here is "parity unpinned".
+ * non-finite voxels in a render (S24); P16 mean / standard deviation / median
+ * (closed forms, numpy float64 moments, np.sort rank); P17 8-bit frame (every byte,
+ * ties, clamps, against the float64 formula).  No function here is "parity
+ * unpinned"; all pins are self-consistency pins (the paper prints no number).
  *
  * Build: gcc -O2 -fopenmp -mfma -ffp-contract=off -shared -fPIC vr_oracle.c -lm
  */
