@@ -364,6 +364,7 @@ def run_ours(args, rig=None, cfg=None):
     images = {m: rig.dev_empty((cfg.height, cfg.width, 4) if m == vr.VR_EA else (cfg.height, cfg.width)) for m in modes}
 
     ev_pairs = []                                    # (start, end) around every vr_render of the timed region
+    quad_launches = []                               # per timed render: launches that used 16-byte row loads
 
     def step(record=False):
         vol.minmax_histogram(256, out=sbuf, stream=rig.stream_arg)
@@ -377,7 +378,10 @@ def run_ours(args, rig=None, cfg=None):
                 vol.render(c, m, out=images[m], stream=rig.stream_arg)
                 if record:
                     rig.record(b); ev_pairs.append((a, b))
-                n += vol.stats()["kernel_launches"]
+                st = vol.stats()
+                n += st["kernel_launches"]
+                if record:
+                    quad_launches.append(st["quad_launches"])
         return n
 
     def barrier():
@@ -512,6 +516,7 @@ def run_ours(args, rig=None, cfg=None):
                           "mean": k_ms, "max": float(np.max(render_ms))},
             "render_ms_by_view": [round(float(np.mean(render_ms[v::frames_step])), 4) for v in range(frames_step)],
             "render_share_of_step": float(np.sum(render_ms)) / ms_total,
+            "quad_launches_by_view": [int(q) for q in quad_launches[:frames_step]],
             "render_ms_cold": ({"mean": float(np.mean(cold_ms)), "max": float(np.max(cold_ms)),
                                 "note": "one orbit at unseen azimuths, outside the timed region"} if cold_ms else None),
             "effective_hbm_gbs_per_frame": 4.0 * n_vox / (k_ms * 1e-3) / 1e9,

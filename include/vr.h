@@ -292,7 +292,7 @@ typedef struct {
     uint32_t skip_variant;          /* 1: the last render launched the empty-space-skipping kernel variant */
     uint32_t bricks_empty;          /* bricks of a brick-major volume dropped by the last render because their whole value
                                        range has opacity 0 (neither uploaded nor marched) */
-    uint32_t reserved;
+    uint32_t quad_launches;         /* lane-mapped launches of the last render that used 16-byte row loads (VR_OPT_ROW_LOADS) */
     uint64_t macro_cells;           /* macrocells of the skipping grid (0: none built) */
     uint64_t empty_cells;           /* cells whose samples all have opacity 0 under the current transfer function,
                                        as of the last flag pass that has COMPLETED on its stream */

@@ -61,7 +61,7 @@ class vr_stats(C.Structure):
                 ("fragments", C.c_uint64), ("h2d_bytes", C.c_uint64), ("d2h_bytes", C.c_uint64),
                 ("total_kernel_launches", C.c_uint64), ("resident_bytes", C.c_uint64),
                 ("zfast_copy", C.c_uint32), ("skip_variant", C.c_uint32), ("bricks_empty", C.c_uint32),
-                ("reserved", C.c_uint32), ("macro_cells", C.c_uint64),
+                ("quad_launches", C.c_uint32), ("macro_cells", C.c_uint64),
                 ("empty_cells", C.c_uint64)]
 
 

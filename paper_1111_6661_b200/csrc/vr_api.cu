@@ -658,17 +658,17 @@ static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam,
     int rows;
     if (!have_z || n_x == 0) {
         make_lane_map(c, n, 0, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 0), rows, img, pitch_f, st);
+        v->stats.quad_launches += launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 0), rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else if (n_x == 9) {
         make_lane_map(c, n, 2, 0, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 2), rows, img, pitch_f, st);
+        v->stats.quad_launches += launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 2), rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else {
         make_lane_map(c, n, 0, 1, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 0), rows, img, pitch_f, st);
+        v->stats.quad_launches += launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 0), rows, img, pitch_f, st);
         make_lane_map(c, n, 2, 2, v->opt_lag, M, rows);
-        launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 2), rows, img, pitch_f, st);
+        v->stats.quad_launches += launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 2), rows, img, pitch_f, st);
         v->stats.kernel_launches += 2;
     }
     v->stats.path = 7;
@@ -886,7 +886,7 @@ VR_API vr_status vr_render(vr_volume *v, const vr_camera *c, int mode, const vr_
     VR_CUDA(cudaSetDevice(v->device));
     cudaStream_t st = (cudaStream_t)stream;
     v->stats.kernel_launches = 0; v->stats.h2d_bytes = 0; v->stats.d2h_bytes = 0; v->stats.fragments = 0;
-    v->stats.bricks_drawn = v->stats.bricks_culled = v->stats.bricks_empty = 0;
+    v->stats.bricks_drawn = v->stats.bricks_culled = v->stats.bricks_empty = v->stats.quad_launches = 0;
 
     float *img = im->pixels;
     long long pitch_f = (long long)(pitch / 4);

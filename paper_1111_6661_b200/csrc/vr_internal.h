@@ -185,8 +185,9 @@ struct PartK {
     int B, nbx, nby;
 };
 
-// part != nullptr: write per-(ray, owner brick) fragments instead of pixels (no ERT, C.7)
-void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
+// part != nullptr: write per-(ray, owner brick) fragments instead of pixels (no ERT, C.7).  Returns true iff the
+// launch used 16-byte row loads.
+bool launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
                  const MacroK &macro, const PartK *part, bool force_wide, bool quad_loads, int rows, float *image,
                  long long pitch_f, cudaStream_t st);
 void launch_fragment_init(int mode, float *arena, unsigned long long n_frag, int grid, cudaStream_t st);

@@ -296,13 +296,13 @@ k_transpose_xz(const float *__restrict__ in, float *__restrict__ out, int nx, in
 
 }  // namespace
 
-void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
+bool launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int fast, const TfK &tf, const LaneMapK &map,
                  const MacroK &macro, const PartK *part, bool force_wide, bool quad_loads, int rows, float *image,
                  long long pitch_f, cudaStream_t st)
 {
     const int n_lane = map.lane_axis == 0 ? cam.width : cam.height;
     const dim3 g((unsigned)((n_lane + 31) / 32), (unsigned)((rows + kRowsPerCta - 1) / kRowsPerCta));
-    if (g.x == 0 || g.y == 0) return;
+    if (g.x == 0 || g.y == 0) return false;
     const unsigned long long span = (unsigned long long)((fast == 0 ? vol.nz : vol.ny) - 1) * (unsigned long long)vol.sb +
                                     (unsigned long long)((fast == 0 ? vol.ny : vol.nx) - 1) * (unsigned long long)vol.sa +
                                     (unsigned long long)(fast == 0 ? vol.nx : vol.nz);
@@ -329,6 +329,7 @@ void launch_rows(int mode, bool ert, const CamK &cam, const LaneVolK &vol, int f
 #undef VR_L2
 #undef VR_L3
 #undef VR_L4
+    return quad;
 }
 
 void launch_fragment_init(int mode, float *arena, unsigned long long n_frag, int grid, cudaStream_t st)

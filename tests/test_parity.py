@@ -535,6 +535,29 @@ def test_progressive_passes(be, path):
         assert e.value.status == vr.VR_ERR_UNSUPPORTED
 
 
+def test_row_loads_default_follows_the_view(be):
+    """VR_OPT_ROW_LOADS = 2 (default): 16-byte row loads for the launches whose rays can enter through the face
+    perpendicular to the memory-fast axis (oblique views of the orbit: both lateral faces visible), scalar loads for
+    the others; volumes whose fast dimension is not a multiple of 4 never use them.  Results are the same either way
+    (test_16_byte_row_loads); this pins the rule the traffic model (profiles/r2_lane_traffic_model.md) is quoted for."""
+    n = (64, 64, 128)
+    v = W.make_cube(W.Recipe(*n, seed=3))
+    want = {0: 0, 2: 2, 8: 0, 10: 2, 14: 2}                       # orbit of 16 views: view -> launches with quads (axis / oblique)
+    with vr.Volume(be.dev(v), n) as vol:
+        for view, quads in want.items():
+            cam = W.orbit_camera(n, view, 16, 64, 48, step=1.0)
+            render(be, vol, cam, vr.VR_MIP)
+            st = vol.stats()
+            assert st["quad_launches"] == quads, (view, st["quad_launches"], st["kernel_launches"])
+        vol.set_option(vr.VR_OPT_ROW_LOADS, 0)
+        render(be, vol, W.orbit_camera(n, 2, 16, 64, 48, step=1.0), vr.VR_MIP)
+        assert vol.stats()["quad_launches"] == 0
+    n2 = (62, 64, 126)
+    with vr.Volume(be.dev(W.make_cube(W.Recipe(*n2, seed=3))), n2) as vol:
+        render(be, vol, W.orbit_camera(n2, 2, 16, 64, 48, step=1.0), vr.VR_MIP)
+        assert vol.stats()["quad_launches"] == 0
+
+
 def test_mixed_camera_renders(be):
     """A camera whose origins AND directions vary per pixel (neither perspective nor orthographic)."""
     n = (32, 32, 32)
