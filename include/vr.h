@@ -328,12 +328,15 @@ VR_API vr_status vr_get_stats(vr_volume *vol, vr_stats *stats);
  *                       0 for the others (bound by instruction issue); see profiles/r2_lane_traffic_model.md.  Quads
  *                       need a memory-fast dimension that is a multiple of 4 and are not used by the empty-space
  *                       skipping variant.
+ *   VR_OPT_TILE_SHEAR   lane-mapped path: 1 (default): every tile of 32 x 64 pixels shears its rows by its own slope (under
+ *                       perspective the slope that keeps a warp on one voxel row changes several-fold across the image);
+ *                       0: one slope per frame, taken at the image centre.
  *   VR_OPT_FORCE_WIDE   1: the render kernels form 64-bit voxel offsets even for volumes of fewer than 2^32
  *                       voxels (the code the largest volumes run; lets the tests cover it at small size).  Default 0.
  * Errors: VR_ERR_INVALID_ARG (NULL handle, unknown option, value out of range).
  * ------------------------------------------------------------------------------------------ */
 enum { VR_OPT_RENDER_PATH = 1, VR_OPT_ZFAST_COPY = 2, VR_OPT_LANE_LAG = 3, VR_OPT_EMPTY_SKIP = 4, VR_OPT_FORCE_WIDE = 5,
-       VR_OPT_ROW_LOADS = 6 };
+       VR_OPT_ROW_LOADS = 6, VR_OPT_TILE_SHEAR = 7 };
 VR_API vr_status vr_set_option(vr_volume *vol, uint32_t option, int64_t value);
 
 /* Thread-local message of the last failing call on this thread ("" if none). */

@@ -24,7 +24,7 @@ def VR_SUBSAMPLE(stride: int, phase_x: int = 0, phase_y: int = 0) -> int:
     """vr_camera.flags of a progressive pass (include/vr.h)."""
     return (int(stride) << 8) | (int(phase_x) << 16) | (int(phase_y) << 24)
 
-VR_OPT_RENDER_PATH, VR_OPT_ZFAST_COPY, VR_OPT_LANE_LAG, VR_OPT_EMPTY_SKIP, VR_OPT_FORCE_WIDE, VR_OPT_ROW_LOADS = 1, 2, 3, 4, 5, 6
+VR_OPT_RENDER_PATH, VR_OPT_ZFAST_COPY, VR_OPT_LANE_LAG, VR_OPT_EMPTY_SKIP, VR_OPT_FORCE_WIDE, VR_OPT_ROW_LOADS, VR_OPT_TILE_SHEAR = 1, 2, 3, 4, 5, 6, 7
 VR_PATH_AUTO, VR_PATH_RAY_MAJOR = 0, 1
 
 _STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_UNSUPPORTED", 3: "VR_ERR_OUT_OF_MEMORY",

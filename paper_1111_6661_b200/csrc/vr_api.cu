@@ -124,7 +124,7 @@ struct vr_volume {
     float *zfast = nullptr;
     bool zfast_failed = false;                // allocation refused once: not retried
     cudaEvent_t zfast_ev = nullptr;           // recorded after the transposition
-    int opt_path = 0, opt_zcopy = 1, opt_lag = 1, opt_wide = 0, opt_quad = 2;   // vr_set_option
+    int opt_path = 0, opt_zcopy = 1, opt_lag = 1, opt_wide = 0, opt_quad = 2, opt_tile_shear = 1;   // vr_set_option
     Staging staging[kStagingRing];
     int staging_next = 0;
 
@@ -657,17 +657,17 @@ static vr_status render_lanes(vr_volume *v, const vr_camera *c, const CamK &cam,
     LaneMapK M;
     int rows;
     if (!have_z || n_x == 0) {
-        make_lane_map(c, n, 0, 0, v->opt_lag, M, rows);
+        make_lane_map(c, n, 0, 0, v->opt_lag, v->opt_tile_shear, M, rows);
         v->stats.quad_launches += launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 0), rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else if (n_x == 9) {
-        make_lane_map(c, n, 2, 0, v->opt_lag, M, rows);
+        make_lane_map(c, n, 2, 0, v->opt_lag, v->opt_tile_shear, M, rows);
         v->stats.quad_launches += launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 2), rows, img, pitch_f, st);
         v->stats.kernel_launches += 1;
     } else {
-        make_lane_map(c, n, 0, 1, v->opt_lag, M, rows);
+        make_lane_map(c, n, 0, 1, v->opt_lag, v->opt_tile_shear, M, rows);
         v->stats.quad_launches += launch_rows(mode, ert, cam, A, 0, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 0), rows, img, pitch_f, st);
-        make_lane_map(c, n, 2, 2, v->opt_lag, M, rows);
+        make_lane_map(c, n, 2, 2, v->opt_lag, v->opt_tile_shear, M, rows);
         v->stats.quad_launches += launch_rows(mode, ert, cam, Z, 2, tf, M, Mc, part, v->opt_wide != 0, launch_quad(v, c, 2), rows, img, pitch_f, st);
         v->stats.kernel_launches += 2;
     }
@@ -1112,6 +1112,9 @@ VR_API vr_status vr_set_option(vr_volume *v, uint32_t option, int64_t value)
     case VR_OPT_ROW_LOADS:
         VR_REQUIRE(value >= 0 && value <= 2, "VR_OPT_ROW_LOADS: 0 scalar, 1 one 16-byte load per row, 2 auto (got %lld)", (long long)value);
         v->opt_quad = (int)value; return VR_OK;
+    case VR_OPT_TILE_SHEAR:
+        VR_REQUIRE(value == 0 || value == 1, "VR_OPT_TILE_SHEAR: 0 one shear per frame, 1 one per tile (got %lld)", (long long)value);
+        v->opt_tile_shear = (int)value; return VR_OK;
     case VR_OPT_FORCE_WIDE:
         VR_REQUIRE(value == 0 || value == 1, "VR_OPT_FORCE_WIDE: 0 or 1 (got %lld)", (long long)value);
         v->opt_wide = (int)value; return VR_OK;

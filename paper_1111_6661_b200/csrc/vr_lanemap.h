@@ -1,29 +1,100 @@
-// vr_lanemap.h — host-only choice of the pixel-to-lane map of the lane-mapped ray-caster (vr_lanes.cu;
-// SURVEY.md row A4's single-GPU analogue of the paper's scheduler): which image axis the 32
-// lanes of a warp run along and by how much the image rows are sheared, so that the samples a warp takes at
-// equal k lie along the memory-fast axis of the volume copy it reads.  O(1) per frame, plain C++ (no CUDA):
-// tests/lanemap_check.cpp executes it and the kernel's pixel formula on the host and checks that every
-// pixel is rendered exactly once for any camera.  The map never changes results, only speed.
+// vr_lanemap.h — the pixel-to-lane map of the lane-mapped ray-caster (vr_lanes.cu; SURVEY.md row A4's
+// single-GPU analogue of the paper's scheduler): which image axis the 32 lanes of a warp run
+// along and by how much the image rows are sheared, so that the samples a warp takes on one plane of the
+// view's principal axis lie along the memory-fast axis of the volume copy it reads.
+//
+// The image (or the pixel lattice of a progressive pass) is cut into TILES of 32 lanes x kLaneTileH rows.  Inside
+// a tile the rows are sheared by an integer offset off(lane) = floor(sigma lane + 1/2) with the tile's OWN sigma,
+// evaluated at the tile's centre: under perspective the ideal shear changes several-fold across the image (the
+// image lines that map to voxel rows meet in a vanishing point), and a lane that drifts off its voxel row costs
+// a cache line of its own per load.  Any sigma gives a bijection of the tile's pixels (proof at lane_pixel), so
+// the map never changes results, only speed.  Host and device use the SAME functions of this header; it is plain
+// C++ (no CUDA needed): tests/lanemap_check.cpp executes them on the host and checks that every pixel is rendered
+// exactly once for any camera.
 #pragma once
 #include <cmath>
 
 #include "../../include/vr.h"
 
+#if defined(__CUDACC__)
+#define VR_HD __host__ __device__
+#else
+#define VR_HD
+#endif
+
 namespace vr {
 
-// Pixel (lane coordinate p, sheared row qs) is image pixel (p, qs + off(p)) along the lane axis, with
-// off(p) = floor(sigma p + 1/2) evaluated in float32 exactly as below (the kernel uses the same formula).
+constexpr int kLaneTileH = 64;          // rows of a tile
+constexpr int kLaneRowsPerCta = 8;      // warps (sheared rows) of a CTA
+
 struct LaneMapK {
     int lane_axis;      // 0: lanes run along image i (rows are j); 1: lanes run along image j
-    float sigma;        // shear of the rows, |sigma| <= 1
-    int q_lo;           // first sheared row (may be negative)
+    float sigma;        // shear at the image centre, |sigma| <= 1 (used for every tile when per_tile == 0)
+    int per_tile;       // 1: every tile evaluates its own shear (VR_OPT_TILE_SHEAR)
+    int bpt;            // CTAs per tile along the rows: ceil((kLaneTileH + 32) / kLaneRowsPerCta)
     int cls;            // pixels this launch renders: 0 all, 1 those with |d_x| <= |d_z|, 2 those with |d_x| > |d_z|
     int lag;            // 0 off; else a lane more than `lag` base planes ahead of the slowest active lane waits
     int paxis, psign;   // principal axis of the view and the sign of travel along it (progress measure of `lag`)
     int w[3];           // psign on paxis, 0 elsewhere: progress of a sample = w . (ix, iy, iz)
+    int fast;           // memory-fast axis of the volume copy this launch reads (0 or 2)
+    float plane_c;      // the plane coord[paxis] = plane_c on which the shear is evaluated (mid-volume)
 };
 
-inline int lane_row_offset(float sigma, int p) { return (int)floorf(fmaf(sigma, (float)p, 0.5f)); }
+VR_HD inline int lane_row_offset(float sigma, int lane) { return (int)floorf(fmaf(sigma, (float)lane, 0.5f)); }
+
+// Shear that keeps a step along the lane axis, taken on the plane coord[paxis] = plane_c, free of any movement
+// along the in-plane axis that is not the fast one, for the ray through the continuous image point (x, y).
+// With P(x, y) = o + s g, s = (plane_c - o_pa) / g_pa:  dP/dx = ou + s_x g + s du,  s_x = -(ou_pa + s du_pa) / g_pa.
+VR_HD inline float lane_pick(const float *a, int k) { return k == 0 ? a[0] : k == 1 ? a[1] : a[2]; }   // no dynamic indexing
+
+template <typename Cam>
+VR_HD inline float lane_shear_at(const Cam &c, int lane_axis, int paxis, int fast, float plane_c, float x, float y)
+{
+    const int other = 3 - paxis - fast;
+    // the paxis and `other` components of origin, direction and their image derivatives
+    const float ou_p = lane_pick(c.ou, paxis), ov_p = lane_pick(c.ov, paxis), du_p = lane_pick(c.du, paxis), dv_p = lane_pick(c.dv, paxis);
+    const float ou_o = lane_pick(c.ou, other), ov_o = lane_pick(c.ov, other), du_o = lane_pick(c.du, other), dv_o = lane_pick(c.dv, other);
+    const float o_p = lane_pick(c.o0, paxis) + x * ou_p + y * ov_p, g_p = lane_pick(c.d0, paxis) + x * du_p + y * dv_p;
+    const float g_o = lane_pick(c.d0, other) + x * du_o + y * dv_o;
+    if (g_p == 0.0f) return 0.0f;
+    const float s = (plane_c - o_p) / g_p;
+    const float si = -(ou_p + s * du_p) / g_p, sj = -(ov_p + s * dv_p) / g_p;
+    const float Pi = ou_o + si * g_o + s * du_o, Pj = ov_o + sj * g_o + s * dv_o;
+    const float L = lane_axis == 0 ? Pi : Pj, R = lane_axis == 0 ? Pj : Pi;
+    float sg = R != 0.0f ? -L / R : 0.0f;
+    if (!(sg >= -1.0f)) sg = sg < 0.0f ? -1.0f : 0.0f;        // NaN -> 0
+    if (sg > 1.0f) sg = 1.0f;
+    return sg;
+}
+
+// Lattice pixel (li, lj) of lane `lane` of warp `warp` of CTA (bx, by); (-1, -1) if that thread has none.
+// Tile (bx, ty = by / bpt) holds lattice pixels p in [32 bx, 32 bx + 32) x q in [q0, q0 + kLaneTileH), q0 =
+// kLaneTileH ty.  Sheared row r = (by % bpt) kLaneRowsPerCta + warp of the tile holds, for every lane, the pixel
+// q = q0 + r - omax + off(lane) if that lies in the tile, with omin <= off(lane) <= omax (off is monotone in the
+// lane and off(0) = 0).  For a fixed lane, r -> q is a shift, and r ranges over [0, kLaneTileH + omax - omin), which
+// contains [omax - off, omax - off + kLaneTileH): every q of the tile is produced exactly once.
+// sub, sx, sy: the lattice of a progressive pass (image pixel = sub * lattice pixel + (sx, sy)); 1, 0, 0 otherwise.
+// rows_of_tile: how many sheared rows of this tile hold pixels (the same for every thread of the tile's CTAs).
+template <typename Cam>
+VR_HD inline void lane_pixel(const Cam &c, const LaneMapK &M, int sub, int sx, int sy, int bx, int by, int warp, int lane,
+                             int &li, int &lj, int &rows_of_tile)
+{
+    const int ty = by / M.bpt, r = (by % M.bpt) * kLaneRowsPerCta + warp, q0 = ty * kLaneTileH;
+    float sigma = M.sigma;
+    if (M.per_tile) {
+        const float pc = (float)(bx * 32 + 16), qc = (float)(q0 + kLaneTileH / 2);      // tile centre, lattice coordinates
+        const float lx = M.lane_axis == 0 ? pc : qc, ly = M.lane_axis == 0 ? qc : pc;
+        sigma = lane_shear_at(c, M.lane_axis, M.paxis, M.fast, M.plane_c, lx * (float)sub + (float)sx, ly * (float)sub + (float)sy);
+    }
+    const int o31 = lane_row_offset(sigma, 31), omax = o31 > 0 ? o31 : 0, omin = o31 < 0 ? o31 : 0;
+    rows_of_tile = kLaneTileH + omax - omin;
+    li = lj = -1;
+    if (r >= rows_of_tile) return;
+    const int p = bx * 32 + lane, q = q0 + r - omax + lane_row_offset(sigma, lane);
+    if (q < q0 || q >= q0 + kLaneTileH) return;
+    li = M.lane_axis == 0 ? p : q;
+    lj = M.lane_axis == 0 ? q : p;
+}
 
 // point where the ray of pixel centre (x, y) (continuous pixel coordinates, C.1 in double) meets the plane
 // `coord[paxis] = c`; false if the ray is parallel to it
@@ -40,8 +111,9 @@ inline bool lane_plane_point(const vr_camera *cam, double x, double y, int paxis
     return std::isfinite(P[0]) && std::isfinite(P[1]) && std::isfinite(P[2]);
 }
 
-// fast: 0 = x-fastest array, 2 = z-fastest copy.  cls as in LaneMapK.  rows = sheared rows to launch.
-inline void make_lane_map(const vr_camera *cam, const int n[3], int fast, int cls, int lag, LaneMapK &M, int &rows)
+// fast: 0 = x-fastest array, 2 = z-fastest copy.  cls as in LaneMapK.  `cam` is the camera of the pixels this launch
+// renders (the lattice camera of a progressive pass).  rows = sheared rows to launch (grid.y * kLaneRowsPerCta).
+inline void make_lane_map(const vr_camera *cam, const int n[3], int fast, int cls, int lag, int per_tile, LaneMapK &M, int &rows)
 {
     const int W = (int)cam->width, H = (int)cam->height;
     const double xc = 0.5 * W, yc = 0.5 * H;
@@ -60,7 +132,10 @@ inline void make_lane_map(const vr_camera *cam, const int n[3], int fast, int cl
     for (int a = 0; a < 3; ++a) M.w[a] = a == pa ? M.psign : 0;
     M.cls = cls;
     M.lag = lag;
-    const int other = 3 - pa - fast;                                  // the in-plane axis that is not the fast one
+    M.fast = fast;
+    M.per_tile = per_tile;
+    M.plane_c = 0.5f * (float)n[pa];
+    M.bpt = (kLaneTileH + 32 + kLaneRowsPerCta - 1) / kLaneRowsPerCta;
     M.lane_axis = 0;
     M.sigma = 0.0f;
     double P0[3], Pi[3], Pj[3];
@@ -69,18 +144,10 @@ inline void make_lane_map(const vr_camera *cam, const int n[3], int fast, int cl
         lane_plane_point(cam, xc, yc + 1.0, pa, c, Pj)) {
         for (int a = 0; a < 3; ++a) { Pi[a] -= P0[a]; Pj[a] -= P0[a]; }
         M.lane_axis = std::fabs(Pi[fast]) >= std::fabs(Pj[fast]) ? 0 : 1;
-        const double *L = M.lane_axis == 0 ? Pi : Pj, *R = M.lane_axis == 0 ? Pj : Pi;
-        // one lane step plus sigma row steps must not move along `other`
-        double s = R[other] != 0.0 ? -L[other] / R[other] : 0.0;
-        if (!std::isfinite(s)) s = 0.0;
-        s = s > 1.0 ? 1.0 : s < -1.0 ? -1.0 : s;
-        M.sigma = (float)s;
+        M.sigma = lane_shear_at(*cam, M.lane_axis, pa, fast, M.plane_c, (float)xc, (float)yc);
     }
-    const int Pn = M.lane_axis == 0 ? W : H, Qn = M.lane_axis == 0 ? H : W;
-    const int o0 = lane_row_offset(M.sigma, 0), o1 = lane_row_offset(M.sigma, Pn > 0 ? Pn - 1 : 0);
-    const int omin = (o0 < o1 ? o0 : o1) - 1, omax = (o0 < o1 ? o1 : o0) + 1;   // one row of slack each side
-    M.q_lo = -omax;                                                   // q = qs + off in [0, Qn)  =>  qs in [-omax, Qn - 1 - omin]
-    rows = Qn - omin + omax;
+    const int Qn = M.lane_axis == 0 ? H : W;
+    rows = (Qn + kLaneTileH - 1) / kLaneTileH * M.bpt * kLaneRowsPerCta;
 }
 
 }  // namespace vr

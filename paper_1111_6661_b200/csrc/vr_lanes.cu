@@ -27,7 +27,7 @@ namespace vr {
 
 namespace {
 
-constexpr int kRowsPerCta = 8, kLaneThreads = 32 * kRowsPerCta;
+constexpr int kRowsPerCta = kLaneRowsPerCta, kLaneThreads = 32 * kRowsPerCta;
 
 // transfer function in shared memory as two float2 tables ((r,g) and (b,a)); entry 256 = copy of 255
 struct TfS { float2 rg[257], ba[257]; };
@@ -174,15 +174,15 @@ __global__ void __launch_bounds__(kLaneThreads)
 k_rows(CamK cam, LaneVolK V, TfK tf, LaneMapK M, MacroK Mc, PartK P, float *__restrict__ image, long long pitch_f)
 {
     __shared__ TfS tf_s;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // pixel of this lane (vr_lanemap.h): tiles of 32 lanes x kLaneTileH rows, each sheared by its own sigma
+    int li, lj, rows_of_tile;
+    lane_pixel(cam, M, cam.sub, cam.sx, cam.sy, (int)blockIdx.x, (int)blockIdx.y, warp, lane, li, lj, rows_of_tile);
+    if (((int)blockIdx.y % M.bpt) * kLaneRowsPerCta >= rows_of_tile) return;    // a CTA beyond the tile's sheared rows (CTA-uniform)
     if (MODE == VR_EA) stage_tf_pairs(tf_s, tf);
     // exact empty-space skipping (vr_macro.cu): used only when enough cells are empty under this transfer function
     const bool skipping = SKIP && __ldg(Mc.n_skip) >= Mc.min_skip;
     const int cxy = Mc.cx * Mc.cy;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // pixel of this lane: p along the lane axis, q = sheared row + off(p)
-    const int p = blockIdx.x * 32 + lane;
-    const int q = M.q_lo + (int)blockIdx.y * kRowsPerCta + warp + __float2int_rd(__fmaf_rn(M.sigma, (float)p, 0.5f));
-    const int li = M.lane_axis == 0 ? p : q, lj = M.lane_axis == 0 ? q : p;      // pixel of the (sub-)lattice
     const bool inside = li >= 0 && li < cam.width && lj >= 0 && lj < cam.height;
     const int i = li * cam.sub + cam.sx, j = lj * cam.sub + cam.sy;              // image pixel (C.1 uses these)
     Ray r;

@@ -1,5 +1,5 @@
-// Host brute force of the pixel-to-lane map of the lane-mapped ray-caster (csrc/vr_lanemap.h + the pixel
-// formula of k_rows in csrc/vr_lanes.cu): for random perspective, orthographic and mixed cameras and image
+// Host brute force of the pixel-to-lane map of the lane-mapped ray-caster (csrc/vr_lanemap.h: make_lane_map and
+// lane_pixel, the function k_rows itself calls): for random perspective, orthographic and mixed cameras and image
 // sizes, every pixel of the image is produced by exactly one (CTA, warp, lane) of the launched grid, for
 // both volume copies and every pixel class.  Also reports how well the shear follows the fast axis.
 #include <cmath>
@@ -36,25 +36,26 @@ int main(int argc, char **argv)
         const int n[3] = { 64, 48, 80 };
         for (int fast = 0; fast <= 2; fast += 2)
             for (int cls = 0; cls <= 2; ++cls) {
+                for (int per_tile = 0; per_tile <= 1; ++per_tile) {
                 LaneMapK M;
                 int rows;
-                make_lane_map(&c, n, fast, cls, 1, M, rows);
+                make_lane_map(&c, n, fast, cls, 1, per_tile, M, rows);
                 const int W = (int)c.width, H = (int)c.height;
                 const int P = M.lane_axis == 0 ? W : H;
                 std::vector<int> cnt((size_t)W * H, 0);
-                const int gx = (P + 31) / 32, gy = (rows + 7) / 8;
-                if (!(M.sigma >= -1.0f && M.sigma <= 1.0f) || M.paxis == fast || M.paxis < 0 || M.paxis > 2) ++bad;
+                const int gx = (P + 31) / 32, gy = rows / kLaneRowsPerCta;
+                if (!(M.sigma >= -1.0f && M.sigma <= 1.0f) || M.paxis == fast || M.paxis < 0 || M.paxis > 2 || rows % kLaneRowsPerCta) ++bad;
                 for (int by = 0; by < gy; ++by)
                     for (int bx = 0; bx < gx; ++bx)
-                        for (int t = 0; t < 256; ++t) {
-                            const int lane = t & 31, warp = t >> 5;
-                            const int p = bx * 32 + lane;
-                            const int q = M.q_lo + by * 8 + warp + lane_row_offset(M.sigma, p);
-                            const int i = M.lane_axis == 0 ? p : q, j = M.lane_axis == 0 ? q : p;
+                        for (int t = 0; t < 32 * kLaneRowsPerCta; ++t) {
+                            int i, j, rt;
+                            lane_pixel(c, M, 1, 0, 0, bx, by, t >> 5, t & 31, i, j, rt);      // the kernel's own pixel formula
+                            if (rt < kLaneTileH || rt > kLaneTileH + 32) ++bad;
                             if (i >= 0 && i < W && j >= 0 && j < H) cnt[(size_t)j * W + i]++;
                         }
                 for (int v : cnt) if (v != 1) ++bad;
                 ++cams;
+                }
             }
     }
     // the configs' own images and orbit cameras (workload/cameras.py): 1024^2, 1920x1080, 3840x2160, 8 views each
@@ -84,16 +85,15 @@ int main(int argc, char **argv)
             for (int fast = 0; fast <= 2; fast += 2) {
                 LaneMapK M;
                 int rows;
-                make_lane_map(&cam, n, fast, fast == 0 ? 1 : 2, 1, M, rows);
+                make_lane_map(&cam, n, fast, fast == 0 ? 1 : 2, 1, 1, M, rows);
                 const int P = M.lane_axis == 0 ? W : H;
                 std::vector<unsigned char> cnt((size_t)W * H, 0);
-                const int gx = (P + 31) / 32, gy = (rows + 7) / 8;
+                const int gx = (P + 31) / 32, gy = rows / kLaneRowsPerCta;
                 for (int by = 0; by < gy; ++by)
                     for (int bx = 0; bx < gx; ++bx)
-                        for (int t = 0; t < 256; ++t) {
-                            const int p = bx * 32 + (t & 31);
-                            const int q = M.q_lo + by * 8 + (t >> 5) + lane_row_offset(M.sigma, p);
-                            const int i = M.lane_axis == 0 ? p : q, j = M.lane_axis == 0 ? q : p;
+                        for (int t = 0; t < 32 * kLaneRowsPerCta; ++t) {
+                            int i, j, rt;
+                            lane_pixel(cam, M, 1, 0, 0, bx, by, t >> 5, t & 31, i, j, rt);
                             if (i >= 0 && i < W && j >= 0 && j < H) cnt[(size_t)j * W + i]++;
                         }
                 for (unsigned char v : cnt) if (v != 1) ++bad;
