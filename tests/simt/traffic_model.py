@@ -29,7 +29,8 @@ SCALE = {2: 1 / 8, 3: 1 / 16, 4: 1 / 16}
 
 
 def run(cfg, v, cam, mode, variant):
-    path, zcopy, lag = variant
+    path, zcopy, lag = variant[:3]
+    tile = variant[3] if len(variant) > 3 else 1
     lib = simt_lib.lib()
     with simt_lib.emulated():
         d = simt_lib.Buffer.of(v, device=True)
@@ -37,6 +38,7 @@ def run(cfg, v, cam, mode, variant):
             vol.set_option(vr.VR_OPT_RENDER_PATH, path)
             vol.set_option(vr.VR_OPT_ZFAST_COPY, zcopy)
             vol.set_option(vr.VR_OPT_LANE_LAG, lag)
+            vol.set_option(vr.VR_OPT_TILE_SHEAR, tile)
             vol.set_option(vr.VR_OPT_EMPTY_SKIP, 0)
             vol.set_option(vr.VR_OPT_ROW_LOADS, 0)                   # the trace counts the scalar loads (+ the quad what-if)
             vol.set_transfer_function(W.tf_haze(cfg.dims, cfg.step), -6.0, 24.0)
@@ -56,6 +58,7 @@ def main():
     variants = [("ray-major 8x4-pixel warps (path 1)", (1, 1, 1)),
                 ("lane-mapped, x-fastest array only, lag 1", (0, 0, 1)),
                 ("lane-mapped + z-fastest copy, lag 0 (no lane synchronisation)", (0, 1, 0)),
+                ("lane-mapped + z-fastest copy, lag 1, one shear per frame", (0, 1, 1, 0)),
                 ("lane-mapped + z-fastest copy, lag 1 (default)", (0, 1, 1)),
                 ("lane-mapped + z-fastest copy, lag 4", (0, 1, 4))]
     print("# Memory-traffic model of the corner loads (host emulation of the library's kernels)\n")
