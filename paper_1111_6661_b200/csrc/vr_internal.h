@@ -48,10 +48,10 @@ inline void vr_launch(void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, 
 #endif
 // memory-traffic model of the emulation (tests/simt/traffic_model.py): addresses of the four row pointers of a sample
 #ifdef VR_SIMT_HOST
-#define VR_TRACE_CORNER_LOADS(active, base, p0, p1, p2, p3) \
-    do { if (::simt::g_trace) ::simt::trace_corner_loads(active, base, p0, p1, p2, p3); } while (0)
+#define VR_TRACE_CORNER_LOADS(sampled, loads, base, p0, p1, p2, p3) \
+    do { if (::simt::g_trace) ::simt::trace_corner_loads(sampled, loads, base, p0, p1, p2, p3); } while (0)
 #else
-#define VR_TRACE_CORNER_LOADS(active, base, p0, p1, p2, p3) ((void)0)
+#define VR_TRACE_CORNER_LOADS(sampled, loads, base, p0, p1, p2, p3) ((void)0)
 #endif
 enum { VR_CNT_LEAP_CELL = 0, VR_CNT_LEAP_BLOCK = 1, VR_CNT_LEAP_REJECTED = 2, VR_CNT_LAG_WAIT = 3, VR_CNT_FRAG_OUTSIDE = 4,
        VR_CNT_FRAG_NO_BRICK = 5 };

@@ -36,6 +36,7 @@ struct LaneMapK {
     int lag;            // 0 off; else a lane more than `lag` base planes ahead of the slowest active lane waits
     int paxis, psign;   // principal axis of the view and the sign of travel along it (progress measure of `lag`)
     int w[3];           // psign on paxis, 0 elsewhere: progress of a sample = w . (ix, iy, iz)
+    int reuse;          // 1: keep a ray's 8 corner voxels in registers while its samples stay in one cell (step < 1 voxel)
     int fast;           // memory-fast axis of the volume copy this launch reads (0 or 2)
     float plane_c;      // the plane coord[paxis] = plane_c on which the shear is evaluated (mid-volume)
 };
@@ -134,6 +135,7 @@ inline void make_lane_map(const vr_camera *cam, const int n[3], int fast, int cl
     M.lag = lag;
     M.fast = fast;
     M.per_tile = per_tile;
+    M.reuse = cam->step < 0.75f ? 1 : 0;
     M.plane_c = 0.5f * (float)n[pa];
     M.bpt = (kLaneTileH + 32 + kLaneRowsPerCta - 1) / kLaneRowsPerCta;
     M.lane_axis = 0;

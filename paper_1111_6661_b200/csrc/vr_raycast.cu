@@ -46,7 +46,7 @@ __device__ __forceinline__ float sample_at(const VolK &V, const Ray &r, float t)
     if (WIDE) p = V.base + ((long long)iz * V.sz + (long long)iy * V.sy + ix);
     else p = V.base + ((unsigned int)iz * (unsigned int)V.sz + (unsigned int)iy * (unsigned int)V.sy + (unsigned int)ix);
     const float *pz = p + V.sz;
-    VR_TRACE_CORNER_LOADS(true, V.base, p, p + V.sy, pz, pz + V.sy);
+    VR_TRACE_CORNER_LOADS(true, true, V.base, p, p + V.sy, pz, pz + V.sy);
     const float v000 = __ldg(p), v100 = __ldg(p + 1);
     const float v010 = __ldg(p + V.sy), v110 = __ldg(p + V.sy + 1);
     const float v001 = __ldg(pz), v101 = __ldg(pz + 1);

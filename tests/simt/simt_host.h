@@ -111,8 +111,8 @@ extern unsigned long long g_counters[16];  // VR_TEST_COUNT(i) of vr_internal.h
 // lane of the warp deposits the addresses of its four row pointers; per load instruction the distinct 128-byte lines
 // and 32-byte sectors (relative to `base`, which is 256-byte aligned on hardware) of the active lanes are counted
 extern int g_trace;
-extern unsigned long long g_trace_stats[8];  // warp iterations, active lanes, load instructions, lines, sectors
-void trace_corner_loads(bool active, const void *base, const void *p0, const void *p1, const void *p2, const void *p3);
+extern unsigned long long g_trace_stats[8];  // warp iterations, sampling lanes, load instructions, lines, sectors, (quad what-if) loads, lines, loading lanes
+void trace_corner_loads(bool sampled, bool loads, const void *base, const void *p0, const void *p1, const void *p2, const void *p3);
 
 struct KernelBody { void (*fn)(void *); void *ctx; };
 void launch_cta_grid(dim3 grid, dim3 block, size_t dyn_smem, KernelBody body);

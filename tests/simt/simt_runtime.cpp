@@ -228,17 +228,26 @@ const WarpTable &warp_exchange(uint32_t mask, uint64_t value)
     return w.table[(my_gen + 1) & 1u];
 }
 
-void trace_corner_loads(bool active, const void *base, const void *p0, const void *p1, const void *p2, const void *p3)
+// sampled: the lane takes a sample in this warp iteration; loads: it also loads the sample's 8 voxels (it may still hold them)
+void trace_corner_loads(bool sampled, bool loads, const void *base, const void *p0, const void *p1, const void *p2, const void *p3)
 {
     const void *ptr[4] = { p0, p1, p2, p3 };
     const int lane = g_running & 31;
+    const uint64_t kIdle = ~0ull, kNoLoad = ~0ull - 1;
     for (int r = 0; r < 4; ++r) {
-        const uint64_t off = active ? (uint64_t)((const char *)ptr[r] - (const char *)base) : ~0ull;
-        const WarpTable &t = warp_exchange(0u, off);                 // every live lane of the warp arrives here
-        int first = -1, n_act = 0;
-        for (int l = 0; l < 32; ++l) if ((t.present >> l & 1u) && t.v[l] != ~0ull) { if (first < 0) first = l; ++n_act; }
+        const uint64_t off = !sampled ? kIdle : !loads ? kNoLoad : (uint64_t)((const char *)ptr[r] - (const char *)base);
+        const WarpTable &t0 = warp_exchange(0u, off);                // every live lane of the warp arrives here
+        WarpTable t = t0;
+        int first = -1, n_smp = 0, n_ld = 0;
+        for (int l = 0; l < 32; ++l) {
+            if (!(t.present >> l & 1u) || t.v[l] == kIdle) { t.v[l] = ~0ull; continue; }
+            if (first < 0) first = l;
+            ++n_smp;
+            if (t.v[l] == kNoLoad) t.v[l] = ~0ull; else ++n_ld;      // below, ~0 = takes no part in the loads
+        }
         if (lane != first) continue;                                 // one lane does the counting
-        if (r == 0) { g_trace_stats[0] += 1; g_trace_stats[1] += (unsigned long long)n_act; }
+        if (r == 0) { g_trace_stats[0] += 1; g_trace_stats[1] += (unsigned long long)n_smp; g_trace_stats[7] += (unsigned long long)n_ld; }
+        if (n_ld == 0) continue;
         for (int e = 0; e < 2; ++e) {                                // the loads of p and p + 1 element
             uint64_t lines[32], sectors[32];
             int nl = 0, ns = 0;

@@ -45,7 +45,7 @@ def run(cfg, v, cam, mode, variant):
             out = simt_lib.Buffer((cam.height, cam.width, 4) if mode == vr.VR_EA else (cam.height, cam.width))
             lib.simt_trace(1)
             vol.render(cam, mode, out=out, stream=0)
-            st = [lib.simt_trace_stat(i) for i in range(7)]
+            st = [lib.simt_trace_stat(i) for i in range(8)]
             lib.simt_trace(0)
     return st
 
@@ -69,27 +69,29 @@ def main():
           "spacing in voxels — what decides coalescing — is the config's own).\n")
     print("`lines / sample` = 8 loads x lines per load / active lanes: the L1 cost of one sample.  `what-if 16 B` = the same with "
           "ONE aligned 16-byte load per row (+ a scalar load for the lanes whose x is the last element of its quad) instead of "
-          "two scalar loads: what `k_rows<QUAD>` (VR_OPT_ROW_LOADS) does, counted from the scalar trace.\n")
-    print("| config (scale) | view | variant | samples | lane efficiency | lines / load | sectors / load | lines / sample | what-if 16 B: lines / sample |")
-    print("|---|---|---|---:|---:|---:|---:|---:|---:|")
+          "two scalar loads: what `k_rows<QUAD>` (VR_OPT_ROW_LOADS) does, counted from the scalar trace.  `samples that load`: "
+          "with a step below one voxel a ray keeps the 8 voxels of its cell in registers, and a sample in the same cell as the ray's "
+          "previous one loads nothing (lane-mapped kernel only).\n")
+    print("| config (scale) | view | variant | samples | lane efficiency | lines / load | sectors / load | lines / sample | what-if 16 B: lines / sample | samples that load |")
+    print("|---|---|---|---:|---:|---:|---:|---:|---:|---:|")
     for number in (int(x) for x in args.configs.split(",")):
         cfg = W.get_config(number, scale=SCALE[number])
         v = W.make_cube(cfg.recipe)
         mode = vr.VR_EA if "ea" in cfg.modes else vr.VR_MIP
         views = list(range(0, cfg.n_views, max(1, cfg.n_views // args.views)))[: args.views]
-        totals = {name: np.zeros(7) for name, _ in variants}
+        totals = {name: np.zeros(8) for name, _ in variants}
         for view in views:
             cam = cfg.camera(view).with_(flags=0)
             for name, var in variants:
                 st = np.array(run(cfg, v, cam, mode, var), dtype=np.float64)
                 totals[name] += st
-                it, act, ld, ln, sc, qld, qln = st
+                it, act, ld, ln, sc, qld, qln, nld = st
                 print(f"| cfg{number} ({SCALE[number]:g}) | {view} | {name} | {int(act)} | {act / (32 * it):.2f} | {ln / ld:.2f} | "
-                      f"{sc / ld:.2f} | {ln / act:.2f} | {qln / act:.2f} |")
+                      f"{sc / ld:.2f} | {ln / act:.2f} | {qln / act:.2f} | {nld / act:.2f} |")
         for name, _ in variants:
-            it, act, ld, ln, sc, qld, qln = totals[name]
+            it, act, ld, ln, sc, qld, qln, nld = totals[name]
             print(f"| **cfg{number} all views** | | **{name}** | {int(act)} | **{act / (32 * it):.2f}** | **{ln / ld:.2f}** | "
-                  f"**{sc / ld:.2f}** | **{ln / act:.2f}** | **{qln / act:.2f}** |")
+                  f"**{sc / ld:.2f}** | **{ln / act:.2f}** | **{qln / act:.2f}** | {nld / act:.2f} |")
 
 
 if __name__ == "__main__":
